@@ -1,0 +1,256 @@
+/* hcc.h — C ABI of the B200-native hierarchy-cut-code ray-reordering hot path.
+ *
+ * Paper: "Faster Ray Tracing through Hierarchy Cut Code", arxiv 2305.16652
+ * (cited as PAPER.md:<line>).  The path (Figure 11; pre-process
+ * :155-192):  density + cut selection -> key computation -> sort of ray indices ->
+ * trace through the sorted indices.  Every step runs in CUDA kernels written for
+ * sm_100a; there is no CPU fallback.
+ *
+ * Conventions
+ *  - Every function returns an int32 status: HCC_OK (0) or a negative hcc_status.
+ *    Nothing throws or aborts across this boundary; hcc_last_error() returns the
+ *    calling thread's last message.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *    Calls that take a stream only ENQUEUE work on it and return; they never
+ *    allocate or free device memory.  Allocation happens in *_create only.
+ *  - "dev" pointers are device pointers owned by the caller (e.g. torch tensors);
+ *    "host" pointers are host memory read during the call.  Handles (hcc_bvh,
+ *    hcc_cut) are owned by the library and released with *_destroy.
+ *  - Alignment: rays 32 bytes; keys, perm, hits, density, workspace 16 bytes.
+ *    A misaligned pointer returns HCC_ERR_BAD_ALIGNMENT.
+ *  - n = 0 is valid everywhere and is a no-op.
+ *
+ * Layouts
+ *  - node (canonical BVH, 32 bytes): { float lo[3], hi[3]; uint32 left_or_first;
+ *    uint32 count }.  count == 0: internal, children are nodes left_or_first and
+ *    left_or_first + 1 (siblings adjacent, parent index < child index, root = 0).
+ *    count > 0: leaf holding triangles prim_idx[left_or_first .. +count), count <= 8.
+ *  - triangle: 9 floats v0 v1 v2; prim ids index this array.
+ *  - ray (32 bytes, AoS): { ox, oy, oz, tmin, dx, dy, dz, tmax }.  d should be unit
+ *    length for TwoPoint (PAPER.md:241 fixed-length estimate); traversal and HCC do
+ *    not require it.
+ *  - key: uint32 when the cut's / call's key_bits <= 32, else uint64; right-aligned
+ *    (all bits above bits_used are zero).
+ *  - closest hit (16 bytes): { float t; uint32 prim; float u; float v }, t = +inf and
+ *    prim = 0xFFFFFFFF on a miss.   any hit: one uint8 per ray (1 = occluded).
+ */
+#ifndef HCC_H
+#define HCC_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Exported symbols (the library is built with -fvisibility=hidden). */
+#if defined(__GNUC__)
+#define HCC_API __attribute__((visibility("default")))
+#else
+#define HCC_API
+#endif
+
+#define HCC_MAX_LEVELS 16u
+#define HCC_MAX_WIDTH 64u
+#define HCC_MISS_PRIM 0xFFFFFFFFu
+
+typedef enum hcc_status {
+    HCC_OK = 0,
+    HCC_ERR_INVALID_ARG = -1,
+    HCC_ERR_BAD_ALIGNMENT = -2,
+    HCC_ERR_OUT_OF_MEMORY = -3,
+    HCC_ERR_CUDA = -4,
+    HCC_ERR_UNSUPPORTED = -5
+} hcc_status;
+
+typedef enum hcc_trace_mode { HCC_TRACE_CLOSEST = 0, HCC_TRACE_ANY = 1 } hcc_trace_mode;
+
+/* The three ray orders compared throughout the paper's Tables 2-3. */
+typedef enum hcc_order { HCC_ORDER_NOSORT = 0, HCC_ORDER_TWOPOINT = 1, HCC_ORDER_HCC = 2 } hcc_order;
+
+typedef struct hcc_node {
+    float lo[3];
+    float hi[3];
+    uint32_t left_or_first;
+    uint32_t count;
+} hcc_node;
+
+typedef struct hcc_hit {
+    float t;
+    uint32_t prim;
+    float u;
+    float v;
+} hcc_hit;
+
+typedef struct hcc_bvh hcc_bvh; /* opaque: device copy of the BVH in the GPU layouts */
+typedef struct hcc_cut hcc_cut; /* opaque: device level tables of one cut hierarchy  */
+typedef struct hcc_pipeline hcc_pipeline; /* opaque: per-batch scratch (keys, perm, sort workspace) */
+
+/* Message of the last error on the calling thread ("" if none). Never NULL. */
+HCC_API const char *hcc_last_error(void);
+
+/* Library version (major*10000 + minor*100 + patch). */
+HCC_API int32_t hcc_version(void);
+
+/* ---- BVH ---------------------------------------------------------------------------
+ * The BVH is INPUT (BASELINE.json north_star: built by a deterministic host binned-SAH
+ * builder); the paper assumes a SAH BVH and does not describe a builder.
+ * hcc_bvh_create validates the canonical arrays on the host (indices in range, siblings
+ * adjacent, parent < child, every node reachable once, leaf count in 1..8, depth <= 63:
+ * otherwise HCC_ERR_INVALID_ARG / HCC_ERR_UNSUPPORTED), copies them to the device and runs
+ * the conversion kernels on `stream`: the 32-byte traversal records (sibling pairs
+ * contiguous and 64-byte aligned), the 48-byte triangle records in leaf order, parent
+ * links and sub-tree leaf counts.  All three arrays are host pointers, read before return.
+ * The call synchronises `stream` before returning. */
+HCC_API int32_t hcc_bvh_create(const hcc_node *nodes_host, uint32_t n_nodes, const float *tris_host,
+                       uint32_t n_tris, const uint32_t *prim_idx_host, void *stream,
+                       hcc_bvh **out);
+HCC_API int32_t hcc_bvh_destroy(hcc_bvh *bvh);
+/* Any out pointer may be NULL.  scene_lo/hi = the root box. */
+HCC_API int32_t hcc_bvh_info(const hcc_bvh *bvh, uint32_t *n_nodes, uint32_t *n_tris, uint32_t *n_leaves,
+                     uint32_t *max_depth, float scene_lo[3], float scene_hi[3]);
+
+/* ---- (a1) density + cut selection ------------------------------------------------------
+ * hcc_density: hierarchically accumulated density, Eq. 1 (:187):
+ *   leaf  HAD = TC * SA;  internal  HAD = (HAD_left + HAD_right) + lambda * SA,
+ *   SA = 2((dx*dy + dy*dz) + dz*dx), every operation one rounded fp32 operation.
+ * density_dev: float32[n_nodes], written.  The paper uses lambda = 0.125 (:185, :276). */
+HCC_API int32_t hcc_density(const hcc_bvh *bvh, float lambda, float *density_dev, void *stream);
+
+/* A cut handle with room for hierarchies of up to max_K finest-level nodes. */
+HCC_API int32_t hcc_cut_create(uint32_t max_K, hcc_cut **out);
+HCC_API int32_t hcc_cut_destroy(hcc_cut *cut);
+
+/* hcc_select_cut: the K-node cut of the BVH by priority-queue search on `density_dev`
+ * (Algorithm 2; cut nodes ordered by density descending, :192), stored
+ * as the level tables the encoder reads.  K <= key_bits gives one level = plain HCC
+ * (:146-153, :206).  K > key_bits gives the multi-level compressed code (:204-237): the
+ * fewest levels m >= 2 of power-of-two widths, the exponent of K split as evenly as
+ * possible (larger first), with sum(widths) <= key_bits; K = (key_bits/2)^2 is the paper's
+ * two-level MLHCC (:216, :220).  If no split fits, K is halved until one does; the K
+ * actually used is reported by hcc_cut_info.  Each table is built by Algorithm 3 (:222-231)
+ * started at its parent entry, with "large enough sub-tree" = at least as many leaves as the
+ * next level's width; a node that is not large enough is kept as an entry (not dropped).
+ * Ties in density break toward the lower node index.
+ * key_bits must be one of 16, 24, 32, 48, 64; K >= 1; else HCC_ERR_INVALID_ARG.
+ * density_dev: float32[n_nodes] (read).  Results stay on the device. */
+HCC_API int32_t hcc_select_cut(const hcc_bvh *bvh, const float *density_dev, uint32_t K, uint32_t key_bits,
+                       hcc_cut *cut, void *stream);
+/* Same with explicit level widths (each 1..64, m <= HCC_MAX_LEVELS, sum <= key_bits). */
+HCC_API int32_t hcc_select_cut_levels(const hcc_bvh *bvh, const float *density_dev, const uint32_t *widths_host,
+                              uint32_t m, uint32_t key_bits, hcc_cut *cut, void *stream);
+/* Shape of the last selection (host values, no synchronisation): number of levels, their
+ * widths (array of HCC_MAX_LEVELS), K actually used, key bits used = sum of widths, key
+ * container bits (32 or 64), total entries and tables over all levels. Out pointers may be NULL. */
+HCC_API int32_t hcc_cut_info(const hcc_cut *cut, uint32_t *m, uint32_t *widths, uint32_t *K_eff,
+                     uint32_t *bits_used, uint32_t *container_bits, uint64_t *n_entries,
+                     uint64_t *n_tables);
+/* Copy the tables to the host for inspection: entry_node_host[n_entries] (node ids, levels
+ * concatenated, table t of level l at offset ent_off[l] + t*w[l], 0xFFFFFFFF = empty slot)
+ * and table_cnt_host[n_tables].  Synchronises `stream`. */
+HCC_API int32_t hcc_cut_read(const hcc_cut *cut, uint32_t *entry_node_host, uint32_t *table_cnt_host,
+                     void *stream);
+
+/* Algorithm 2 verbatim for ANY K, as its data-parallel closed form:
+ * because the density of a parent is >= that of its children and popping a leaf never
+ * advances the loop, the cut is the set of children of the K-1 highest-density internal
+ * nodes that are not themselves among those K-1 (ties -> lower index).  Implemented as a
+ * radix sort of the internal nodes by density plus a flag/compact pass and a final sort by
+ * density (:192).  cut_nodes_dev: uint32[K] written with the node ids, density descending;
+ * count_dev: uint32[1] = number written = min(K, #leaves).  workspace from
+ * hcc_select_cut_flat_workspace_bytes. */
+HCC_API int32_t hcc_select_cut_flat_workspace_bytes(const hcc_bvh *bvh, uint32_t K, uint64_t *bytes);
+HCC_API int32_t hcc_select_cut_flat(const hcc_bvh *bvh, const float *density_dev, uint32_t K,
+                            uint32_t *cut_nodes_dev, uint32_t *count_dev, void *workspace_dev,
+                            uint64_t workspace_bytes, void *stream);
+
+/* ---- (a2) encode ----------------------------------------------------------------------
+ * hcc_encode: the hierarchy cut code of every ray (Algorithm 1; levels
+ * below the first :208, :218-220).  Bit for entry j of a level = [ray hits that node's
+ * box], entry 0 (highest density) in the field's most significant bit (:192, :202); the top
+ * level's field is the most significant, each further level directly below (:216, :220);
+ * the representative of a level is its first hit entry (:218); a level with no hit zeroes
+ * all lower fields.  Box test: inv = 1/d; t1 = (lo-o)*inv, t2 = (hi-o)*inv per axis,
+ * tn = max(tmin, max_a min(t1,t2)), tf = min(tmax, min_a max(t1,t2)), hit <=> tn <= tf,
+ * IEEE fp32 operation by operation with NaN-dropping min/max.
+ * keys_dev: uint32[n] if the cut's container is 32 bits, else uint64[n]. */
+HCC_API int32_t hcc_encode(const float *rays_dev, uint64_t n, const hcc_cut *cut, void *keys_dev, void *stream);
+
+/* TwoPoint comparison path: origin and estimated end point
+ * o + (0.25 * largest scene extent) * d, each coordinate quantised to floor(key_bits/6)
+ * bits inside [scene_lo, scene_hi] and bit-interleaved o.x o.y o.z t.x t.y t.z from the
+ * most significant bit down.  keys_dev: uint32[n] if key_bits <= 32 else uint64[n]. */
+HCC_API int32_t hcc_encode_twopoint(const float *rays_dev, uint64_t n, const float scene_lo[3],
+                            const float scene_hi[3], uint32_t key_bits, void *keys_dev, void *stream);
+
+/* ---- (a3) sort ------------------------------------------------------------------------
+ * Stable ascending order of ray ids by key ("sorting the HCCs as natural
+ * numbers", :247 "sorts the indices of rays"): perm_dev[j] = id of the ray at rank j; equal
+ * keys keep ascending id.  LSD radix sort, 8-bit digits, one chained-scan ("onesweep") pass
+ * per digit over bits [0, bits_used); bits above bits_used must be zero.
+ * keys_dev (container_bits = 32 or 64) is clobbered.  n < 2^30.
+ * workspace_dev: at least hcc_sort_workspace_bytes(n, container_bits) bytes. */
+HCC_API int32_t hcc_sort_workspace_bytes(uint64_t n, uint32_t container_bits, uint64_t *bytes);
+HCC_API int32_t hcc_sort(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bits_used,
+                 uint32_t *perm_dev, void *workspace_dev, uint64_t workspace_bytes, void *stream);
+
+/* ---- (a4) trace -----------------------------------------------------------------------
+ * Thread j traces ray perm_dev[j] (perm_dev == NULL: ray j, the NoSort order) and writes
+ * the result at the ray's own index ("the trace kernel fetches the rays based
+ * on these sorted indices").  CLOSEST: hits_dev = hcc_hit[n]: the triangle with the
+ * smallest t in (tmin, tmax), ties to the lowest prim id.  ANY: hits_dev = uint8[n].
+ * Triangle test (fp32, fmaf where written): e1 = v1-v0, e2 = v2-v0, p = d x e2,
+ * det = e1.p (0 -> miss), inv = 1/det, s = o-v0, u = (s.p)*inv, q = s x e1, v = (d.q)*inv,
+ * t = (e2.q)*inv; hit <=> u >= 0, v >= 0, u+v <= 1, tmin < t < tmax; with
+ * cross(a,b).x = fmaf(a.y,b.z,-(a.z*b.y)) and dot(a,b) = fmaf(a.x,b.x,fmaf(a.y,b.y,a.z*b.z)). */
+HCC_API int32_t hcc_trace(const hcc_bvh *bvh, const float *rays_dev, uint64_t n, const uint32_t *perm_dev,
+                  int32_t mode, void *hits_dev, void *stream);
+
+/* Same traversal, instrumented (never used for timing): stats_dev = uint64[4], zeroed by the
+ * call, then [0] = sibling pairs fetched (64 bytes each), [1] = triangle records fetched
+ * (48 bytes each), [2] = rays traced, [3] = deepest traversal stack.  hits_dev as hcc_trace. */
+HCC_API int32_t hcc_trace_stats(const hcc_bvh *bvh, const float *rays_dev, uint64_t n, const uint32_t *perm_dev,
+                        int32_t mode, void *hits_dev, uint64_t *stats_dev, void *stream);
+
+/* ---- the per-batch path as one call -----------------------------------------------------
+ * PAPER.md:245-247 (Figure 11): key compute kernel -> ray sort kernel -> trace kernel, per
+ * ray batch.  A pipeline handle owns the scratch for batches of up to n_max rays (keys, perm,
+ * the sort workspace, and with host_staging != 0 a device copy of the rays and hits), so a
+ * call allocates nothing.  container_bits_max: 32 or 64 = widest key it must hold. */
+HCC_API int32_t hcc_pipeline_create(uint64_t n_max, uint32_t container_bits_max, uint32_t host_staging,
+                            hcc_pipeline **out);
+HCC_API int32_t hcc_pipeline_destroy(hcc_pipeline *p);
+
+/* Enqueue encode + sort + trace of one batch on `stream` (device pointers).
+ *  order HCC_ORDER_HCC:      keys = hcc_encode(rays, cut);               `cut` required
+ *  order HCC_ORDER_TWOPOINT: keys = hcc_encode_twopoint(rays, root box, key_bits); cut ignored
+ *  order HCC_ORDER_NOSORT:   no keys, no sort; rays traced in input order
+ * then perm = hcc_sort(keys) and hcc_trace(bvh, rays, perm, mode, hits_dev).
+ * perm_out_dev: NULL, or uint32[n] that receives the permutation (untouched for NOSORT).
+ * key_bits is used by TWOPOINT only. */
+HCC_API int32_t hcc_reorder_trace(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
+                          uint32_t key_bits, const float *rays_dev, uint64_t n, int32_t mode,
+                          void *hits_dev, uint32_t *perm_out_dev, void *stream);
+/* The same with HOST buffers: copies rays_host (32 n bytes; pinned memory makes the copy
+ * asynchronous) to the device, runs the batch, copies the hits (16 n bytes CLOSEST, n bytes
+ * ANY) to hits_host and synchronises `stream` before returning.  Needs host_staging. */
+HCC_API int32_t hcc_reorder_trace_host(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
+                               uint32_t key_bits, const float *rays_host, uint64_t n, int32_t mode,
+                               void *hits_host, void *stream);
+/* Device time of the stages of the pipeline's last call, from CUDA events recorded on its
+ * stream between the stages: ms[0] encode, [1] sort, [2] trace, [3] host->device copy,
+ * [4] device->host copy (3, 4 = 0 for the device form).  Waits for that call to finish. */
+HCC_API int32_t hcc_pipeline_stage_ms(hcc_pipeline *p, float ms[5]);
+
+/* ANC, "average number of codes per warp" (Table 7): for every group of 32
+ * consecutive ranks j (the rays one traversal warp holds) the number of distinct keys
+ * keys_dev[perm_dev[j]] (perm_dev NULL = identity).  out_dev = uint64[2], zeroed by the call:
+ * [0] = sum over warps of distinct keys, [1] = number of warps.  keys_dev is in ORIGINAL ray
+ * order (hcc_sort clobbers its input: pass a copy made before sorting). */
+HCC_API int32_t hcc_anc(const void *keys_dev, const uint32_t *perm_dev, uint64_t n, uint32_t container_bits,
+                uint64_t *out_dev, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HCC_H */

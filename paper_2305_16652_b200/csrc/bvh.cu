@@ -1,0 +1,250 @@
+// BVH upload + GPU layout conversion, and (a1) hierarchically accumulated density
+// (Eq. 1 at :187).  Compiled with -fmad=false: every source-level
+// floating-point operation is one IEEE fp32 operation.
+#include <stdarg.h>
+#include <string.h>
+
+#include <vector>
+
+#include "common.cuh"
+
+namespace hcc {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+}
+
+// ---------------------------------------------------------------------------------------
+// conversion kernels
+// ---------------------------------------------------------------------------------------
+
+// Traversal record of node i, stored at record index i+1 so that a sibling pair
+// (left odd in the canonical numbering) starts on a 64-byte boundary:
+//   rec[2*(i+1)+0] = (lo.x, lo.y, lo.z, ref)      rec[2*(i+1)+1] = (hi.x, hi.y, hi.z, 0)
+//   ref, internal: record index of the left child = left + 1   (bit 31 clear)
+//   ref, leaf    : 0x80000000 | (count-1) << 28 | first triangle slot
+__global__ void k_convert_nodes(const hcc_node *__restrict__ nodes, uint32_t n, float4 *__restrict__ rec,
+                                uint32_t *__restrict__ parent) {
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    hcc_node nd = nodes[i];
+    uint32_t ref;
+    if (nd.count == 0) {
+        ref = nd.left_or_first + 1u;
+        parent[nd.left_or_first] = i;
+        parent[nd.left_or_first + 1u] = i;
+    } else {
+        ref = 0x80000000u | ((nd.count - 1u) << 28) | nd.left_or_first;
+    }
+    if (i == 0) parent[0] = 0xFFFFFFFFu;
+    rec[2 * (size_t)(i + 1) + 0] = make_float4(nd.lo[0], nd.lo[1], nd.lo[2], __uint_as_float(ref));
+    rec[2 * (size_t)(i + 1) + 1] = make_float4(nd.hi[0], nd.hi[1], nd.hi[2], 0.0f);
+    if (i == 0) {  // record 0 is padding
+        rec[0] = make_float4(0.f, 0.f, 0.f, 0.f);
+        rec[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+
+// Triangle record k (leaf order): (v0, prim id), (e1 = v1 - v0, 0), (e2 = v2 - v0, 0).
+__global__ void k_convert_tris(const float *__restrict__ tris, const uint32_t *__restrict__ prim_idx,
+                               uint32_t n, float4 *__restrict__ out) {
+    uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    uint32_t id = prim_idx[k];
+    const float *v = tris + 9 * (size_t)id;
+    float v0x = v[0], v0y = v[1], v0z = v[2];
+    out[3 * (size_t)k + 0] = make_float4(v0x, v0y, v0z, __uint_as_float(id));
+    out[3 * (size_t)k + 1] = make_float4(v[3] - v0x, v[4] - v0y, v[5] - v0z, 0.0f);
+    out[3 * (size_t)k + 2] = make_float4(v[6] - v0x, v[7] - v0y, v[8] - v0z, 0.0f);
+}
+
+// Bottom-up pass: one thread per leaf walks to the root; at each parent the second
+// thread to arrive continues (both children are final by then).  Computes the number
+// of leaves below every node.
+__global__ void k_subtree_leaves(const hcc_node *__restrict__ nodes, const uint32_t *__restrict__ parent,
+                                 uint32_t *flags, uint32_t n, uint32_t *leaves) {
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n || nodes[i].count == 0) return;
+    leaves[i] = 1u;
+    uint32_t cur = i;
+    while (cur != 0u) {
+        uint32_t p = parent[cur];
+        __threadfence();
+        if (atomicAdd(&flags[p], 1u) == 0u) return;
+        uint32_t l = nodes[p].left_or_first;
+        leaves[p] = __ldcg(&leaves[l]) + __ldcg(&leaves[l + 1u]);
+        cur = p;
+    }
+}
+
+__device__ __forceinline__ float surface_area(const hcc_node &nd) {
+    float dx = nd.hi[0] - nd.lo[0];
+    float dy = nd.hi[1] - nd.lo[1];
+    float dz = nd.hi[2] - nd.lo[2];
+    return 2.0f * ((dx * dy + dy * dz) + dz * dx);
+}
+
+// Eq. 1, same bottom-up schedule.  Each node's value is computed exactly
+// once from its two final children, so the result does not depend on thread timing.
+__global__ void k_density(const hcc_node *__restrict__ nodes, const uint32_t *__restrict__ parent,
+                          uint32_t *flags, uint32_t n, float lambda, float *had) {
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    hcc_node nd = nodes[i];
+    if (nd.count == 0) return;
+    had[i] = (float)nd.count * surface_area(nd);
+    uint32_t cur = i;
+    while (cur != 0u) {
+        uint32_t p = parent[cur];
+        __threadfence();
+        if (atomicAdd(&flags[p], 1u) == 0u) return;
+        hcc_node pn = nodes[p];
+        float hl = __ldcg(&had[pn.left_or_first]);
+        float hr = __ldcg(&had[pn.left_or_first + 1u]);
+        had[p] = (hl + hr) + (lambda * surface_area(pn));
+        cur = p;
+    }
+}
+
+}  // namespace hcc
+
+using namespace hcc;
+
+extern "C" const char *hcc_last_error(void) { return hcc::g_err; }
+extern "C" int32_t hcc_version(void) { return 100; }
+
+extern "C" int32_t hcc_bvh_destroy(hcc_bvh *b) {
+    if (!b) return HCC_OK;
+    cudaFree(b->d_nodes);
+    cudaFree(b->d_parent);
+    cudaFree(b->d_leaves);
+    cudaFree(b->d_flags);
+    cudaFree(b->d_internal);
+    cudaFree(b->d_trec);
+    cudaFree(b->d_ttri);
+    delete b;
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_bvh_create(const hcc_node *nodes, uint32_t n_nodes, const float *tris, uint32_t n_tris,
+                                  const uint32_t *prim_idx, void *stream, hcc_bvh **out) {
+    HCC_REQUIRE(nodes && tris && prim_idx && out, HCC_ERR_INVALID_ARG, "hcc_bvh_create: NULL argument");
+    HCC_REQUIRE(n_nodes >= 1 && n_tris >= 1, HCC_ERR_INVALID_ARG, "hcc_bvh_create: empty BVH");
+    HCC_REQUIRE(n_tris < (1u << 28) && n_nodes < (1u << 30), HCC_ERR_UNSUPPORTED,
+                "hcc_bvh_create: more than 2^28 triangles or 2^30 nodes");
+    *out = nullptr;
+    cudaStream_t s = (cudaStream_t)stream;
+
+    // ---- host validation: one pass in index order (parent < child makes depth a prefix computation)
+    std::vector<uint32_t> depth(n_nodes, 0u);
+    std::vector<uint8_t> seen(n_nodes, 0), tri_seen(n_tris, 0);
+    std::vector<uint32_t> internal_ids;
+    internal_ids.reserve(n_nodes / 2 + 1);
+    uint32_t max_depth = 0, n_leaves = 0;
+    uint64_t tri_total = 0;
+    seen[0] = 1;
+    for (uint32_t i = 0; i < n_nodes; ++i) {
+        const hcc_node &nd = nodes[i];
+        HCC_REQUIRE(seen[i], HCC_ERR_INVALID_ARG, "hcc_bvh_create: node %u is not reachable from the root", i);
+        if (depth[i] > max_depth) max_depth = depth[i];
+        if (nd.count == 0) {
+            uint32_t l = nd.left_or_first;
+            internal_ids.push_back(i);
+            HCC_REQUIRE(l > i && (uint64_t)l + 1u < n_nodes, HCC_ERR_INVALID_ARG,
+                        "hcc_bvh_create: node %u has children out of range or not after it", i);
+            HCC_REQUIRE(!seen[l] && !seen[l + 1], HCC_ERR_INVALID_ARG, "hcc_bvh_create: node %u shares a child", i);
+            seen[l] = seen[l + 1] = 1;
+            depth[l] = depth[l + 1] = depth[i] + 1u;
+        } else {
+            ++n_leaves;
+            HCC_REQUIRE(nd.count <= 8u, HCC_ERR_UNSUPPORTED, "hcc_bvh_create: leaf %u holds %u > 8 triangles", i, nd.count);
+            HCC_REQUIRE((uint64_t)nd.left_or_first + nd.count <= n_tris, HCC_ERR_INVALID_ARG,
+                        "hcc_bvh_create: leaf %u triangle range out of bounds", i);
+            tri_total += nd.count;
+        }
+    }
+    for (uint32_t k = 0; k < n_tris; ++k) {
+        HCC_REQUIRE(prim_idx[k] < n_tris, HCC_ERR_INVALID_ARG, "hcc_bvh_create: prim_idx[%u] out of range", k);
+        tri_seen[prim_idx[k]] = 1;
+    }
+    HCC_REQUIRE(max_depth <= 63u, HCC_ERR_UNSUPPORTED, "hcc_bvh_create: BVH depth %u > 63", max_depth);
+    (void)tri_total;
+
+    hcc_bvh *b = new hcc_bvh();
+    memset(b, 0, sizeof *b);
+    b->n_nodes = n_nodes; b->n_tris = n_tris; b->n_leaves = n_leaves; b->max_depth = max_depth;
+    for (int a = 0; a < 3; ++a) { b->scene_lo[a] = nodes[0].lo[a]; b->scene_hi[a] = nodes[0].hi[a]; }
+
+    float *d_tris = nullptr;
+    uint32_t *d_prim = nullptr;
+    cudaError_t e = cudaSuccess;
+    auto alloc = [&](void **p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
+    alloc((void **)&b->d_nodes, sizeof(hcc_node) * (size_t)n_nodes);
+    alloc((void **)&b->d_parent, sizeof(uint32_t) * (size_t)n_nodes);
+    alloc((void **)&b->d_leaves, sizeof(uint32_t) * (size_t)n_nodes);
+    alloc((void **)&b->d_flags, sizeof(uint32_t) * (size_t)n_nodes);
+    alloc((void **)&b->d_internal, sizeof(uint32_t) * (internal_ids.size() + 1));
+    alloc((void **)&b->d_trec, sizeof(float4) * 2 * ((size_t)n_nodes + 1));
+    alloc((void **)&b->d_ttri, sizeof(float4) * 3 * (size_t)n_tris);
+    alloc((void **)&d_tris, sizeof(float) * 9 * (size_t)n_tris);
+    alloc((void **)&d_prim, sizeof(uint32_t) * (size_t)n_tris);
+    if (e != cudaSuccess) {
+        set_error("hcc_bvh_create: cudaMalloc failed: %s", cudaGetErrorString(e));
+        cudaFree(d_tris); cudaFree(d_prim);
+        hcc_bvh_destroy(b);
+        return e == cudaErrorMemoryAllocation ? HCC_ERR_OUT_OF_MEMORY : HCC_ERR_CUDA;
+    }
+    auto fail = [&](cudaError_t err, const char *what) {
+        set_error("hcc_bvh_create: %s: %s", what, cudaGetErrorString(err));
+        cudaFree(d_tris); cudaFree(d_prim);
+        hcc_bvh_destroy(b);
+        return (int32_t)HCC_ERR_CUDA;
+    };
+    if ((e = cudaMemcpyAsync(b->d_nodes, nodes, sizeof(hcc_node) * (size_t)n_nodes, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy nodes");
+    if ((e = cudaMemcpyAsync(d_tris, tris, sizeof(float) * 9 * (size_t)n_tris, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy triangles");
+    if ((e = cudaMemcpyAsync(d_prim, prim_idx, sizeof(uint32_t) * (size_t)n_tris, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy prim_idx");
+    if (!internal_ids.empty() &&
+        (e = cudaMemcpyAsync(b->d_internal, internal_ids.data(), sizeof(uint32_t) * internal_ids.size(), cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy internal ids");
+    if ((e = cudaMemsetAsync(b->d_flags, 0, sizeof(uint32_t) * (size_t)n_nodes, s)) != cudaSuccess) return fail(e, "memset");
+    const uint32_t T = 256;
+    k_convert_nodes<<<(n_nodes + T - 1) / T, T, 0, s>>>(b->d_nodes, n_nodes, b->d_trec, b->d_parent);
+    k_convert_tris<<<(n_tris + T - 1) / T, T, 0, s>>>(d_tris, d_prim, n_tris, b->d_ttri);
+    k_subtree_leaves<<<(n_nodes + T - 1) / T, T, 0, s>>>(b->d_nodes, b->d_parent, b->d_flags, n_nodes, b->d_leaves);
+    if ((e = cudaGetLastError()) != cudaSuccess) return fail(e, "conversion kernels");
+    if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return fail(e, "synchronise");
+    cudaFree(d_tris);
+    cudaFree(d_prim);
+    *out = b;
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_bvh_info(const hcc_bvh *b, uint32_t *n_nodes, uint32_t *n_tris, uint32_t *n_leaves,
+                                uint32_t *max_depth, float scene_lo[3], float scene_hi[3]) {
+    HCC_REQUIRE(b, HCC_ERR_INVALID_ARG, "hcc_bvh_info: NULL bvh");
+    if (n_nodes) *n_nodes = b->n_nodes;
+    if (n_tris) *n_tris = b->n_tris;
+    if (n_leaves) *n_leaves = b->n_leaves;
+    if (max_depth) *max_depth = b->max_depth;
+    for (int a = 0; a < 3; ++a) {
+        if (scene_lo) scene_lo[a] = b->scene_lo[a];
+        if (scene_hi) scene_hi[a] = b->scene_hi[a];
+    }
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_density(const hcc_bvh *b, float lambda, float *density_dev, void *stream) {
+    HCC_REQUIRE(b && density_dev, HCC_ERR_INVALID_ARG, "hcc_density: NULL argument");
+    HCC_REQUIRE(aligned(density_dev, 16), HCC_ERR_BAD_ALIGNMENT, "hcc_density: density_dev not 16-byte aligned");
+    HCC_REQUIRE(lambda >= 0.0f, HCC_ERR_INVALID_ARG, "hcc_density: lambda must be >= 0");
+    cudaStream_t s = (cudaStream_t)stream;
+    HCC_CUDA_TRY(cudaMemsetAsync(b->d_flags, 0, sizeof(uint32_t) * (size_t)b->n_nodes, s));
+    const uint32_t T = 256;
+    k_density<<<(b->n_nodes + T - 1) / T, T, 0, s>>>(b->d_nodes, b->d_parent, b->d_flags, b->n_nodes, lambda, density_dev);
+    HCC_CUDA_TRY(cudaGetLastError());
+    return HCC_OK;
+}

@@ -1,0 +1,89 @@
+// Shared host/device helpers of the CUDA path (sm_100a).  Nothing here is used by the
+// oracle; the two share no code.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/hcc.h"
+
+namespace hcc {
+
+void set_error(const char *fmt, ...);
+
+#define HCC_CUDA_TRY(expr)                                                              \
+    do {                                                                                \
+        cudaError_t _e = (expr);                                                        \
+        if (_e != cudaSuccess) {                                                        \
+            hcc::set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e),      \
+                           __FILE__, __LINE__);                                         \
+            return HCC_ERR_CUDA;                                                        \
+        }                                                                               \
+    } while (0)
+
+#define HCC_REQUIRE(cond, status, ...)                                                  \
+    do {                                                                                \
+        if (!(cond)) {                                                                  \
+            hcc::set_error(__VA_ARGS__);                                                \
+            return (status);                                                            \
+        }                                                                               \
+    } while (0)
+
+inline bool aligned(const void *p, uintptr_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) == 0; }
+
+inline int sm_count() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
+            n = 148;
+    }
+    return n;
+}
+
+inline uint64_t round_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
+
+// Device-side level tables of a cut hierarchy, passed to kernels by value.
+struct CutDev {
+    uint32_t m;                        // number of levels
+    uint32_t w[HCC_MAX_LEVELS];        // level widths
+    uint32_t ent_off[HCC_MAX_LEVELS];  // first entry of level l in the flat arrays
+    uint32_t tab_off[HCC_MAX_LEVELS];  // first table of level l
+    uint32_t n_tab[HCC_MAX_LEVELS];    // tables on level l = prod(w[0..l-1])
+    uint32_t n_entries;                // sum over levels of n_tab*w
+    uint32_t n_tables;
+    uint32_t bits_used;
+    const float4 *boxes;               // 2 float4 per entry: (lo.xyz, cnt-of-table in entry 0), (hi.xyz, -)
+    const uint32_t *entry_node;
+    const uint32_t *table_cnt;
+};
+
+}  // namespace hcc
+
+struct hcc_bvh {
+    uint32_t n_nodes, n_tris, n_leaves, max_depth;
+    float scene_lo[3], scene_hi[3];
+    hcc_node *d_nodes;      // canonical nodes
+    uint32_t *d_parent;     // parent index (root: 0xFFFFFFFF)
+    uint32_t *d_leaves;     // sub-tree leaf counts
+    uint32_t *d_flags;      // arrival counters of the bottom-up passes
+    uint32_t *d_internal;   // indices of the internal nodes, ascending
+    float4 *d_trec;         // traversal records: 2 float4 per node at index (i+1)
+    float4 *d_ttri;         // 3 float4 per triangle, leaf order
+    // scratch for hcc_select_cut_flat lives in the caller's workspace
+};
+
+struct hcc_cut {
+    uint32_t cap_entries, cap_tables;
+    uint32_t K_eff, key_bits, container_bits;
+    hcc::CutDev dev;        // pointers into the buffers below
+    float4 *d_boxes;
+    uint32_t *d_entry_node;
+    uint32_t *d_table_cnt;
+    bool valid;
+};
+
+// stage entry points implemented in the other translation units
+namespace hcc {
+int32_t launch_build_tables(const hcc_bvh *bvh, const float *had, hcc_cut *cut, cudaStream_t s);
+}

@@ -1,0 +1,201 @@
+// (a2) key computation: hierarchy cut code (Algorithm 1), its multi-level
+// compressed form (:204-237) and the TwoPoint comparison key (:92, :241).
+// Compiled with -fmad=false: the slab test is the IEEE operation sequence hcc.h states.
+#include "common.cuh"
+
+namespace hcc {
+
+__device__ __forceinline__ float max3(float a, float b, float c) {
+    float d;
+    asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));   // FMNMX3, NaN operands dropped
+    return d;
+}
+__device__ __forceinline__ float min3(float a, float b, float c) {
+    float d;
+    asm("min.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+    return d;
+}
+
+__device__ __forceinline__ float4 ld_stream(const float4 *p) {
+    float4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+    return r;
+}
+
+struct RayEnc {
+    float ox, oy, oz, tmin, ix, iy, iz, tmax;
+};
+
+// Alg. 1 line 5: t1 = (lo - o) * inv, t2 = (hi - o) * inv per axis (subtract, round, multiply,
+// round), tn = max(tmin, max_a min(t1,t2)), tf = min(tmax, min_a max(t1,t2)), hit <=> tn <= tf.
+// min/max drop NaN operands, so the reduction order does not matter.
+__device__ __forceinline__ bool slab_hit(const RayEnc &r, const float4 lo, const float4 hi) {
+    float t1x = (lo.x - r.ox) * r.ix, t2x = (hi.x - r.ox) * r.ix;
+    float t1y = (lo.y - r.oy) * r.iy, t2y = (hi.y - r.oy) * r.iy;
+    float t1z = (lo.z - r.oz) * r.iz, t2z = (hi.z - r.oz) * r.iz;
+    float tn = fmaxf(max3(fminf(t1x, t2x), fminf(t1y, t2y), fminf(t1z, t2z)), r.tmin);
+    float tf = fminf(min3(fmaxf(t1x, t2x), fmaxf(t1y, t2y), fmaxf(t1z, t2z)), r.tmax);
+    return tn <= tf;
+}
+
+// Mask of one table over entries [j0, j1): entry j -> bit (j1-1-j) of the result (<= 32 entries).
+template <bool SMEM>
+__device__ __forceinline__ uint32_t table_mask(const RayEnc &r, const float4 *__restrict__ box, uint32_t j0, uint32_t j1) {
+    uint32_t mask = 0;
+#pragma unroll 4
+    for (uint32_t j = j0; j < j1; ++j) {
+        float4 lo, hi;
+        if (SMEM) { lo = box[2 * j]; hi = box[2 * j + 1]; }
+        else      { lo = __ldg(box + 2 * j); hi = __ldg(box + 2 * j + 1); }
+        mask = (mask << 1) | (slab_hit(r, lo, hi) ? 1u : 0u);
+    }
+    return mask;
+}
+
+constexpr int ENC_THREADS = 256;
+
+// Alg. 1: line 1 "copy cut nodes from global memory into shared memory" (the first
+// smem_entries entries = whole levels), line 2 grid-stride "while have ray", lines 4-6 per
+// level.  One ray per thread per iteration; 32-byte rays read as two 16-byte loads.
+template <typename KeyT>
+__global__ void __launch_bounds__(ENC_THREADS)
+k_encode_hcc(const float4 *__restrict__ rays, uint64_t n, const CutDev cut, uint32_t smem_entries,
+             KeyT *__restrict__ keys) {
+    extern __shared__ float4 s_box[];
+    for (uint32_t i = threadIdx.x; i < 2u * smem_entries; i += ENC_THREADS) s_box[i] = cut.boxes[i];
+    __syncthreads();
+    const uint64_t stride = (uint64_t)gridDim.x * ENC_THREADS;
+    for (uint64_t ri = (uint64_t)blockIdx.x * ENC_THREADS + threadIdx.x; ri < n; ri += stride) {
+        float4 a = ld_stream(rays + 2 * ri), b = ld_stream(rays + 2 * ri + 1);
+        RayEnc r;
+        r.ox = a.x; r.oy = a.y; r.oz = a.z; r.tmin = a.w;
+        r.ix = 1.0f / b.x; r.iy = 1.0f / b.y; r.iz = 1.0f / b.z; r.tmax = b.w;
+        unsigned long long key = 0;
+        uint32_t table = 0;
+        bool alive = true;
+        for (uint32_t l = 0; l < cut.m; ++l) {
+            const uint32_t w = cut.w[l];
+            unsigned long long mask = 0;
+            if (alive) {
+                const uint32_t e0 = cut.ent_off[l] + table * w;
+                const bool in_smem = e0 < smem_entries;           // uniform per level
+                const float4 *box = in_smem ? s_box + 2 * (size_t)e0 : cut.boxes + 2 * (size_t)e0;
+                const uint32_t cnt = __float_as_uint(in_smem ? box[0].w : __ldg(&box[0].w));
+                // entries [0,cnt) are valid; entry j -> bit (w-1-j)
+                uint32_t c_hi = cnt > 32u ? cnt - 32u : 0u;       // only flat tables wider than 32
+                unsigned long long m_hi = 0;
+                if (c_hi) m_hi = in_smem ? table_mask<true>(r, box, 0, c_hi) : table_mask<false>(r, box, 0, c_hi);
+                uint32_t m_lo = in_smem ? table_mask<true>(r, box, c_hi, cnt) : table_mask<false>(r, box, c_hi, cnt);
+                mask = (c_hi ? (m_hi << 32) : 0ull) | (unsigned long long)m_lo;   // cnt bits, entry 0 on top
+                uint32_t rep = (uint32_t)__clzll((long long)mask) - (64u - cnt);  // first hit entry (mask != 0)
+                mask = cnt ? mask << (w - cnt) : 0ull;            // cnt >= 1 keeps the shift below 64
+                if (mask == 0ull) alive = false; else table = table * w + rep;
+            }
+            key = (w < 64u ? key << w : 0ull) | mask;
+        }
+        keys[ri] = (KeyT)key;
+    }
+}
+
+// TwoPoint: quantise o and o + len*d to b bits per coordinate, interleave.
+__device__ __forceinline__ uint32_t quantise(float p, float lo, float hi, float scale, uint32_t qmax) {
+    float ext = hi - lo;
+    if (!(ext > 0.0f)) return 0u;
+    float x = ((p - lo) / ext) * scale;
+    if (!(x >= 0.0f)) return 0u;
+    if (x >= scale) return qmax;
+    return (uint32_t)x;
+}
+
+template <typename KeyT>
+__global__ void __launch_bounds__(ENC_THREADS)
+k_encode_twopoint(const float4 *__restrict__ rays, uint64_t n, float3 lo, float3 hi, float len, uint32_t b,
+                  KeyT *__restrict__ keys) {
+    const uint64_t stride = (uint64_t)gridDim.x * ENC_THREADS;
+    const float scale = (float)(1u << b);
+    const uint32_t qmax = (1u << b) - 1u;
+    for (uint64_t ri = (uint64_t)blockIdx.x * ENC_THREADS + threadIdx.x; ri < n; ri += stride) {
+        float4 o = ld_stream(rays + 2 * ri), d = ld_stream(rays + 2 * ri + 1);
+        uint32_t q[6];
+        q[0] = quantise(o.x, lo.x, hi.x, scale, qmax);
+        q[1] = quantise(o.y, lo.y, hi.y, scale, qmax);
+        q[2] = quantise(o.z, lo.z, hi.z, scale, qmax);
+        q[3] = quantise(o.x + len * d.x, lo.x, hi.x, scale, qmax);
+        q[4] = quantise(o.y + len * d.y, lo.y, hi.y, scale, qmax);
+        q[5] = quantise(o.z + len * d.z, lo.z, hi.z, scale, qmax);
+        unsigned long long key = 0;
+        for (int i = (int)b - 1; i >= 0; --i) {
+#pragma unroll
+            for (int c = 0; c < 6; ++c) key = (key << 1) | ((q[c] >> i) & 1u);
+        }
+        keys[ri] = (KeyT)key;
+    }
+}
+
+static int grid_for(const void *kernel, size_t smem, uint64_t n) {
+    int per_sm = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, ENC_THREADS, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+    uint64_t want = (n + ENC_THREADS - 1) / ENC_THREADS;
+    uint64_t cap = (uint64_t)sm_count() * (uint64_t)per_sm;
+    return (int)(want < cap ? want : cap);
+}
+
+}  // namespace hcc
+
+using namespace hcc;
+
+extern "C" int32_t hcc_encode(const float *rays_dev, uint64_t n, const hcc_cut *cut, void *keys_dev, void *stream) {
+    HCC_REQUIRE(cut && cut->valid, HCC_ERR_INVALID_ARG, "hcc_encode: the cut handle holds no selection");
+    if (n == 0) return HCC_OK;
+    HCC_REQUIRE(rays_dev && keys_dev, HCC_ERR_INVALID_ARG, "hcc_encode: NULL argument");
+    HCC_REQUIRE(aligned(rays_dev, 32) && aligned(keys_dev, 16), HCC_ERR_BAD_ALIGNMENT,
+                "hcc_encode: rays need 32-byte, keys 16-byte alignment");
+    HCC_REQUIRE(n < (1ull << 32), HCC_ERR_UNSUPPORTED, "hcc_encode: n >= 2^32");
+    cudaStream_t s = (cudaStream_t)stream;
+    const CutDev &d = cut->dev;
+    // stage whole levels, top down, while they fit in 160 KB (leaves room for 1 CTA/SM at worst)
+    const size_t budget = 160 * 1024;
+    uint32_t smem_entries = 0;
+    for (uint32_t l = 0; l < d.m; ++l) {
+        uint32_t end = d.ent_off[l] + d.n_tab[l] * d.w[l];
+        if ((size_t)end * 32 <= budget) smem_entries = end; else break;
+    }
+    size_t smem = (size_t)smem_entries * 32;
+    if (cut->container_bits == 32) {
+        auto kern = k_encode_hcc<uint32_t>;
+        HCC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget));
+        kern<<<grid_for((const void *)kern, smem, n), ENC_THREADS, smem, s>>>((const float4 *)rays_dev, n, d, smem_entries, (uint32_t *)keys_dev);
+    } else {
+        auto kern = k_encode_hcc<unsigned long long>;
+        HCC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget));
+        kern<<<grid_for((const void *)kern, smem, n), ENC_THREADS, smem, s>>>((const float4 *)rays_dev, n, d, smem_entries, (unsigned long long *)keys_dev);
+    }
+    HCC_CUDA_TRY(cudaGetLastError());
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_encode_twopoint(const float *rays_dev, uint64_t n, const float scene_lo[3], const float scene_hi[3],
+                                       uint32_t key_bits, void *keys_dev, void *stream) {
+    HCC_REQUIRE(key_bits == 16 || key_bits == 24 || key_bits == 32 || key_bits == 48 || key_bits == 64,
+                HCC_ERR_INVALID_ARG, "hcc_encode_twopoint: key_bits must be 16, 24, 32, 48 or 64");
+    if (n == 0) return HCC_OK;
+    HCC_REQUIRE(rays_dev && keys_dev && scene_lo && scene_hi, HCC_ERR_INVALID_ARG, "hcc_encode_twopoint: NULL argument");
+    HCC_REQUIRE(aligned(rays_dev, 32) && aligned(keys_dev, 16), HCC_ERR_BAD_ALIGNMENT,
+                "hcc_encode_twopoint: rays need 32-byte, keys 16-byte alignment");
+    cudaStream_t s = (cudaStream_t)stream;
+    float3 lo = make_float3(scene_lo[0], scene_lo[1], scene_lo[2]);
+    float3 hi = make_float3(scene_hi[0], scene_hi[1], scene_hi[2]);
+    float e = fmaxf(fmaxf(hi.x - lo.x, hi.y - lo.y), hi.z - lo.z);
+    float len = 0.25f * e;
+    uint32_t b = key_bits / 6u;
+    if (key_bits <= 32) {
+        auto kern = k_encode_twopoint<uint32_t>;
+        kern<<<grid_for((const void *)kern, 0, n), ENC_THREADS, 0, s>>>((const float4 *)rays_dev, n, lo, hi, len, b, (uint32_t *)keys_dev);
+    } else {
+        auto kern = k_encode_twopoint<unsigned long long>;
+        kern<<<grid_for((const void *)kern, 0, n), ENC_THREADS, 0, s>>>((const float4 *)rays_dev, n, lo, hi, len, b, (unsigned long long *)keys_dev);
+    }
+    HCC_CUDA_TRY(cudaGetLastError());
+    return HCC_OK;
+}

@@ -1,0 +1,180 @@
+// The whole per-batch hot path behind one call (Figure 11): key compute
+// kernel -> ray sort kernel -> trace kernel, for the three orderings the bench compares
+// (NoSort, TwoPoint, hierarchy cut code), plus the host-buffer form of the same call and the
+// ANC diagnostic (Table 7).  All scratch lives in the hcc_pipeline handle, so
+// nothing is allocated per batch.
+#include <string.h>
+
+#include "common.cuh"
+
+struct hcc_pipeline {
+    uint64_t n_max;
+    uint32_t container_bits_max;
+    bool host_staging;
+    void *d_keys;
+    uint32_t *d_perm;
+    void *d_ws;
+    uint64_t ws_bytes;
+    float *d_rays;      // host-buffer form only
+    void *d_hits;       // host-buffer form only
+    cudaEvent_t ev[6];  // h2d start, encode start, sort start, trace start, trace end, d2h end
+    bool timed, timed_host;
+};
+
+namespace hcc {
+
+// ANC: number of distinct codes among the 32 rays of each warp, in traced
+// order.  One warp per group of 32 consecutive ranks; out[0] += distinct codes, out[1] += warps.
+template <typename KeyT>
+__global__ void k_anc(const KeyT *__restrict__ keys, const uint32_t *__restrict__ perm, uint32_t n,
+                      unsigned long long *out) {
+    const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool valid = j < n;
+    const uint32_t active = __ballot_sync(0xFFFFFFFFu, valid);
+    if (!valid) return;
+    const KeyT k = keys[perm ? perm[j] : j];
+    const uint32_t peers = __match_any_sync(active, k);
+    const bool leader = (__ffs(peers) - 1) == (int)(threadIdx.x & 31u);
+    const uint32_t distinct = __popc(__ballot_sync(active, leader));
+    if ((threadIdx.x & 31u) == (uint32_t)(__ffs(active) - 1)) {
+        atomicAdd(&out[0], (unsigned long long)distinct);
+        atomicAdd(&out[1], 1ull);
+    }
+}
+
+}  // namespace hcc
+
+using namespace hcc;
+
+extern "C" int32_t hcc_pipeline_destroy(hcc_pipeline *p) {
+    if (!p) return HCC_OK;
+    cudaFree(p->d_keys);
+    cudaFree(p->d_perm);
+    cudaFree(p->d_ws);
+    cudaFree(p->d_rays);
+    cudaFree(p->d_hits);
+    for (int i = 0; i < 6; ++i)
+        if (p->ev[i]) cudaEventDestroy(p->ev[i]);
+    delete p;
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_pipeline_create(uint64_t n_max, uint32_t container_bits_max, uint32_t host_staging,
+                                       hcc_pipeline **out) {
+    HCC_REQUIRE(out, HCC_ERR_INVALID_ARG, "hcc_pipeline_create: NULL out");
+    *out = nullptr;
+    HCC_REQUIRE(n_max >= 1 && n_max < (1ull << 30), HCC_ERR_INVALID_ARG, "hcc_pipeline_create: n_max must be in 1..2^30-1");
+    HCC_REQUIRE(container_bits_max == 32 || container_bits_max == 64, HCC_ERR_INVALID_ARG,
+                "hcc_pipeline_create: container_bits_max must be 32 or 64");
+    hcc_pipeline *p = new hcc_pipeline();
+    memset(p, 0, sizeof *p);
+    p->n_max = n_max;
+    p->container_bits_max = container_bits_max;
+    p->host_staging = host_staging != 0;
+    int32_t rc = hcc_sort_workspace_bytes(n_max, container_bits_max, &p->ws_bytes);
+    if (rc != HCC_OK) { delete p; return rc; }
+    cudaError_t e = cudaMalloc(&p->d_keys, (size_t)(container_bits_max / 8) * n_max);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&p->d_perm, sizeof(uint32_t) * n_max);
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_ws, p->ws_bytes);
+    if (e == cudaSuccess && p->host_staging) e = cudaMalloc((void **)&p->d_rays, 32 * n_max);
+    if (e == cudaSuccess && p->host_staging) e = cudaMalloc(&p->d_hits, 16 * n_max);
+    for (int i = 0; i < 6 && e == cudaSuccess; ++i) e = cudaEventCreate(&p->ev[i]);
+    if (e != cudaSuccess) {
+        set_error("hcc_pipeline_create: %s", cudaGetErrorString(e));
+        hcc_pipeline_destroy(p);
+        return e == cudaErrorMemoryAllocation ? HCC_ERR_OUT_OF_MEMORY : HCC_ERR_CUDA;
+    }
+    *out = p;
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_reorder_trace(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
+                                     uint32_t key_bits, const float *rays_dev, uint64_t n, int32_t mode,
+                                     void *hits_dev, uint32_t *perm_out_dev, void *stream) {
+    HCC_REQUIRE(p && bvh, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: NULL handle");
+    HCC_REQUIRE(order == HCC_ORDER_NOSORT || order == HCC_ORDER_TWOPOINT || order == HCC_ORDER_HCC, HCC_ERR_INVALID_ARG,
+                "hcc_reorder_trace: unknown order %d", order);
+    HCC_REQUIRE(n <= p->n_max, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: n exceeds the pipeline's n_max");
+    cudaStream_t s = (cudaStream_t)stream;
+    uint32_t *perm = perm_out_dev ? perm_out_dev : p->d_perm;
+    int32_t rc = HCC_OK;
+    p->timed = false;
+    HCC_CUDA_TRY(cudaEventRecord(p->ev[1], s));
+    uint32_t container = 32, bits_used = 0;
+    if (order == HCC_ORDER_HCC) {
+        HCC_REQUIRE(cut && cut->valid, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: order HCC needs a selected cut");
+        container = cut->container_bits;
+        bits_used = cut->dev.bits_used;
+        HCC_REQUIRE(container <= p->container_bits_max, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: 64-bit keys in a 32-bit pipeline");
+        rc = hcc_encode(rays_dev, n, cut, p->d_keys, stream);
+    } else if (order == HCC_ORDER_TWOPOINT) {
+        container = key_bits <= 32 ? 32u : 64u;
+        bits_used = 6u * (key_bits / 6u);
+        HCC_REQUIRE(container <= p->container_bits_max, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: 64-bit keys in a 32-bit pipeline");
+        rc = hcc_encode_twopoint(rays_dev, n, bvh->scene_lo, bvh->scene_hi, key_bits, p->d_keys, stream);
+    }
+    if (rc != HCC_OK) return rc;
+    HCC_CUDA_TRY(cudaEventRecord(p->ev[2], s));
+    if (order != HCC_ORDER_NOSORT) {
+        rc = hcc_sort(p->d_keys, n, container, bits_used, perm, p->d_ws, p->ws_bytes, stream);
+        if (rc != HCC_OK) return rc;
+    }
+    HCC_CUDA_TRY(cudaEventRecord(p->ev[3], s));
+    rc = hcc_trace(bvh, rays_dev, n, order == HCC_ORDER_NOSORT ? nullptr : perm, mode, hits_dev, stream);
+    if (rc != HCC_OK) return rc;
+    HCC_CUDA_TRY(cudaEventRecord(p->ev[4], s));
+    p->timed = true;
+    p->timed_host = false;
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_reorder_trace_host(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
+                                          uint32_t key_bits, const float *rays_host, uint64_t n, int32_t mode,
+                                          void *hits_host, void *stream) {
+    HCC_REQUIRE(p && p->host_staging, HCC_ERR_INVALID_ARG, "hcc_reorder_trace_host: pipeline created without host staging");
+    HCC_REQUIRE(n <= p->n_max, HCC_ERR_INVALID_ARG, "hcc_reorder_trace_host: n exceeds the pipeline's n_max");
+    HCC_REQUIRE(mode == HCC_TRACE_CLOSEST || mode == HCC_TRACE_ANY, HCC_ERR_INVALID_ARG, "hcc_reorder_trace_host: unknown mode %d", mode);
+    if (n == 0) return HCC_OK;
+    HCC_REQUIRE(rays_host && hits_host, HCC_ERR_INVALID_ARG, "hcc_reorder_trace_host: NULL argument");
+    cudaStream_t s = (cudaStream_t)stream;
+    HCC_CUDA_TRY(cudaEventRecord(p->ev[0], s));
+    HCC_CUDA_TRY(cudaMemcpyAsync(p->d_rays, rays_host, 32 * n, cudaMemcpyHostToDevice, s));
+    int32_t rc = hcc_reorder_trace(p, bvh, cut, order, key_bits, p->d_rays, n, mode, p->d_hits, nullptr, stream);
+    if (rc != HCC_OK) return rc;
+    HCC_CUDA_TRY(cudaMemcpyAsync(hits_host, p->d_hits, (mode == HCC_TRACE_CLOSEST ? 16 : 1) * n, cudaMemcpyDeviceToHost, s));
+    HCC_CUDA_TRY(cudaEventRecord(p->ev[5], s));
+    HCC_CUDA_TRY(cudaStreamSynchronize(s));
+    p->timed_host = true;
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_pipeline_stage_ms(hcc_pipeline *p, float ms[5]) {
+    HCC_REQUIRE(p && ms, HCC_ERR_INVALID_ARG, "hcc_pipeline_stage_ms: NULL argument");
+    HCC_REQUIRE(p->timed, HCC_ERR_INVALID_ARG, "hcc_pipeline_stage_ms: no completed call to time");
+    HCC_CUDA_TRY(cudaEventSynchronize(p->ev[p->timed_host ? 5 : 4]));
+    for (int i = 0; i < 3; ++i) HCC_CUDA_TRY(cudaEventElapsedTime(&ms[i], p->ev[1 + i], p->ev[2 + i]));
+    ms[3] = ms[4] = 0.0f;
+    if (p->timed_host) {
+        HCC_CUDA_TRY(cudaEventElapsedTime(&ms[3], p->ev[0], p->ev[1]));
+        HCC_CUDA_TRY(cudaEventElapsedTime(&ms[4], p->ev[4], p->ev[5]));
+    }
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_anc(const void *keys_dev, const uint32_t *perm_dev, uint64_t n, uint32_t container_bits,
+                           uint64_t *out_dev, void *stream) {
+    HCC_REQUIRE(container_bits == 32 || container_bits == 64, HCC_ERR_INVALID_ARG, "hcc_anc: container_bits must be 32 or 64");
+    HCC_REQUIRE(out_dev && aligned(out_dev, 16), HCC_ERR_INVALID_ARG, "hcc_anc: out_dev NULL or misaligned");
+    cudaStream_t s = (cudaStream_t)stream;
+    HCC_CUDA_TRY(cudaMemsetAsync(out_dev, 0, 2 * sizeof(uint64_t), s));
+    if (n == 0) return HCC_OK;
+    HCC_REQUIRE(keys_dev, HCC_ERR_INVALID_ARG, "hcc_anc: NULL keys");
+    HCC_REQUIRE(n < (1ull << 32), HCC_ERR_UNSUPPORTED, "hcc_anc: n >= 2^32");
+    const uint32_t T = 256, blocks = (uint32_t)((n + T - 1) / T);
+    if (container_bits == 32)
+        k_anc<uint32_t><<<blocks, T, 0, s>>>((const uint32_t *)keys_dev, perm_dev, (uint32_t)n, (unsigned long long *)out_dev);
+    else
+        k_anc<unsigned long long><<<blocks, T, 0, s>>>((const unsigned long long *)keys_dev, perm_dev, (uint32_t)n, (unsigned long long *)out_dev);
+    HCC_CUDA_TRY(cudaGetLastError());
+    return HCC_OK;
+}

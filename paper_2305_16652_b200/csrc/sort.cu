@@ -1,0 +1,271 @@
+// (a3) sort of (key, ray id) pairs: stable LSD radix sort, 8-bit digits, one chained-scan
+// ("onesweep") kernel per digit with warp match ranking and decoupled look-back.
+// PAPER.md:196 ("sorting the HCCs as natural numbers"), :247 ("sorts the indices of rays").
+// The paper calls Thrust; this is a from-scratch sm_100a kernel family.
+#include "common.cuh"
+
+namespace hcc {
+
+constexpr int RADIX_BITS = 8;
+constexpr int RADIX = 1 << RADIX_BITS;
+constexpr int SORT_THREADS = 256;            // == RADIX: thread d owns digit d in the scan phases
+constexpr int SORT_WARPS = SORT_THREADS / 32;
+constexpr int SORT_ITEMS = 16;
+constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;   // 4096 pairs per CTA
+constexpr int MAX_PASSES = 8;
+constexpr uint32_t FLAG_AGG = 1u << 30, FLAG_PREFIX = 2u << 30, VAL_MASK = (1u << 30) - 1u;
+constexpr int HIST_THREADS = 256;
+
+// control region of the workspace (zeroed once per sort by one memset)
+struct SortCtl {
+    uint32_t hist[MAX_PASSES][RADIX];
+    uint32_t ticket[MAX_PASSES];
+    uint32_t pad[8];
+};
+
+__device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t *p) {
+    uint32_t v;
+    asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void st_volatile_u32(uint32_t *p, uint32_t v) {
+    asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// All digit histograms in one read of the keys.
+template <typename KeyT>
+__global__ void __launch_bounds__(HIST_THREADS)
+k_histogram(const KeyT *__restrict__ keys, uint32_t n, uint32_t passes, SortCtl *ctl) {
+    __shared__ uint32_t sh[MAX_PASSES][RADIX];
+    for (uint32_t i = threadIdx.x; i < MAX_PASSES * RADIX; i += HIST_THREADS) (&sh[0][0])[i] = 0u;
+    __syncthreads();
+    const uint32_t stride = gridDim.x * HIST_THREADS;
+    for (uint32_t i = blockIdx.x * HIST_THREADS + threadIdx.x; i < n; i += stride) {
+        KeyT k = keys[i];
+        for (uint32_t p = 0; p < passes; ++p) atomicAdd(&sh[p][(uint32_t)(k >> (RADIX_BITS * p)) & (RADIX - 1)], 1u);
+    }
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < passes * RADIX; i += HIST_THREADS) {
+        uint32_t c = (&sh[0][0])[i];
+        if (c) atomicAdd(&(&ctl->hist[0][0])[i], c);
+    }
+}
+
+// Exclusive scan of each digit histogram, written as the PREFIX row of "tile -1"
+// (row 0 of that pass's status array), so the look-back needs no special first tile.
+__global__ void __launch_bounds__(RADIX)
+k_scan_hist(const SortCtl *ctl, uint32_t *status, size_t status_stride) {
+    __shared__ uint32_t s_w[RADIX / 32];
+    const uint32_t p = blockIdx.x, d = threadIdx.x, lane = d & 31u, warp = d >> 5;
+    uint32_t v = ctl->hist[p][d], incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if (lane >= (uint32_t)o) incl += x;
+    }
+    if (lane == 31) s_w[warp] = incl;
+    __syncthreads();
+    uint32_t add = 0;
+    for (uint32_t w = 0; w < warp; ++w) add += s_w[w];
+    status[p * status_stride + d] = FLAG_PREFIX | (add + incl - v);
+}
+
+__global__ void k_iota(uint32_t *perm, uint32_t n) {
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) perm[i] = i;
+}
+
+// One radix pass.  status: (tiles + 1) rows of RADIX words for this pass; row t+1 belongs to
+// tile t: empty (0), AGG | count of the tile, or PREFIX | count of tiles 0..t plus the digit's
+// global base.  Tiles are handed out by an atomic ticket so that every predecessor of a
+// running tile is itself running or done (forward progress of the look-back spin).
+template <typename KeyT, bool FIRST, bool WRITE_KEYS>
+__global__ void __launch_bounds__(SORT_THREADS)
+k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const uint32_t *__restrict__ vals_in,
+           uint32_t *__restrict__ vals_out, uint32_t n, uint32_t shift, uint32_t *status, uint32_t *ticket) {
+    __shared__ uint32_t s_warp_hist[SORT_WARPS][RADIX];
+    __shared__ uint32_t s_tile_off[RADIX];
+    __shared__ uint32_t s_gbase[RADIX];
+    __shared__ uint32_t s_warp_tot[SORT_WARPS];
+    __shared__ uint32_t s_tile;
+    extern __shared__ __align__(16) unsigned char s_dyn[];
+    KeyT *s_keys = reinterpret_cast<KeyT *>(s_dyn);
+    uint32_t *s_vals = reinterpret_cast<uint32_t *>(s_dyn + sizeof(KeyT) * SORT_TILE);
+
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
+    for (uint32_t i = tid; i < SORT_WARPS * RADIX; i += SORT_THREADS) (&s_warp_hist[0][0])[i] = 0u;
+    __syncthreads();
+    const uint32_t tile = s_tile;
+    const uint32_t tile_base = tile * SORT_TILE;
+    const uint32_t count = min((uint32_t)SORT_TILE, n - tile_base);
+    const uint32_t my_base = warp * (SORT_ITEMS * 32) + lane;   // item i at my_base + 32*i (warp-striped)
+
+    KeyT key[SORT_ITEMS];
+    uint32_t rank[SORT_ITEMS];
+#pragma unroll
+    for (int i = 0; i < SORT_ITEMS; ++i) {
+        uint32_t idx = my_base + 32 * i;
+        key[i] = idx < count ? keys_in[tile_base + idx] : (KeyT)0;
+    }
+    // rank every item among the equal digits of its warp, in (item, lane) order
+    const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int i = 0; i < SORT_ITEMS; ++i) {
+        const bool valid = my_base + 32 * i < count;
+        const uint32_t digit = valid ? ((uint32_t)(key[i] >> shift) & (RADIX - 1)) : (uint32_t)RADIX;
+        const uint32_t peers = __match_any_sync(0xFFFFFFFFu, digit);
+        const uint32_t below = __popc(peers & lt);
+        const uint32_t old = s_warp_hist[warp][digit & (RADIX - 1)];
+        __syncwarp();
+        if (valid && below == 0) s_warp_hist[warp][digit] = old + __popc(peers);
+        __syncwarp();
+        rank[i] = old + below;
+    }
+    __syncthreads();
+
+    // thread d: digit d.  Warp-exclusive offsets, tile total, publish, scan over digits, look back.
+    {
+        const uint32_t d = tid;
+        uint32_t run = 0;
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; ++w) {
+            uint32_t t = s_warp_hist[w][d];
+            s_warp_hist[w][d] = run;
+            run += t;
+        }
+        const uint32_t total = run;
+        uint32_t *row = status + (size_t)(tile + 1) * RADIX;
+        st_volatile_u32(row + d, FLAG_AGG | total);
+        uint32_t incl = total;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= (uint32_t)o) incl += x;
+        }
+        if (lane == 31) s_warp_tot[warp] = incl;
+        __syncthreads();
+        uint32_t add = 0;
+        for (uint32_t w = 0; w < warp; ++w) add += s_warp_tot[w];
+        const uint32_t excl_local = add + incl - total;
+        s_tile_off[d] = excl_local;
+        // decoupled look-back over rows tile, tile-1, ..., 0 (row 0 = seeded global digit base)
+        uint32_t excl = 0;
+        const uint32_t *prow = status + (size_t)tile * RADIX + d;
+        for (;;) {
+            uint32_t v = ld_volatile_u32(prow);
+            if ((v >> 30) == 0u) continue;
+            excl += v & VAL_MASK;
+            if (v & FLAG_PREFIX) break;
+            prow -= RADIX;
+        }
+        st_volatile_u32(row + d, FLAG_PREFIX | ((excl + total) & VAL_MASK));
+        s_gbase[d] = excl - excl_local;
+    }
+    __syncthreads();
+
+    // scatter into tile order in shared memory
+#pragma unroll
+    for (int i = 0; i < SORT_ITEMS; ++i) {
+        const uint32_t idx = my_base + 32 * i;
+        if (idx < count) {
+            const uint32_t digit = (uint32_t)(key[i] >> shift) & (RADIX - 1);
+            const uint32_t p = s_tile_off[digit] + s_warp_hist[warp][digit] + rank[i];
+            s_keys[p] = key[i];
+            s_vals[p] = FIRST ? tile_base + idx : vals_in[tile_base + idx];
+        }
+    }
+    __syncthreads();
+    // write out: consecutive threads -> consecutive addresses inside each digit run
+    for (uint32_t p = tid; p < count; p += SORT_THREADS) {
+        const KeyT k = s_keys[p];
+        const uint32_t pos = s_gbase[(uint32_t)(k >> shift) & (RADIX - 1)] + p;
+        if (WRITE_KEYS) keys_out[pos] = k;
+        vals_out[pos] = s_vals[p];
+    }
+}
+
+static uint64_t ctl_bytes(uint64_t n) {
+    uint64_t tiles = (n + SORT_TILE - 1) / SORT_TILE;
+    return round_up(sizeof(SortCtl), 256) + round_up((uint64_t)MAX_PASSES * (tiles + 1) * RADIX * sizeof(uint32_t), 256);
+}
+
+template <typename KeyT>
+static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t *perm, unsigned char *ws, cudaStream_t s) {
+    const uint32_t tiles = (n + SORT_TILE - 1) / SORT_TILE;
+    KeyT *keys_tmp = reinterpret_cast<KeyT *>(ws);
+    uint32_t *vals_tmp = reinterpret_cast<uint32_t *>(ws + round_up(sizeof(KeyT) * (uint64_t)n, 256));
+    unsigned char *ctl_raw = ws + round_up(sizeof(KeyT) * (uint64_t)n, 256) + round_up(sizeof(uint32_t) * (uint64_t)n, 256);
+    SortCtl *ctl = reinterpret_cast<SortCtl *>(ctl_raw);
+    uint32_t *status = reinterpret_cast<uint32_t *>(ctl_raw + round_up(sizeof(SortCtl), 256));
+    const size_t status_stride = (size_t)(tiles + 1) * RADIX;
+    HCC_CUDA_TRY(cudaMemsetAsync(ctl_raw, 0, round_up(sizeof(SortCtl), 256) + (size_t)passes * status_stride * sizeof(uint32_t), s));
+    int hist_blocks = (int)((n + HIST_THREADS * 16 - 1) / (HIST_THREADS * 16));
+    int cap = sm_count() * 4;
+    if (hist_blocks > cap) hist_blocks = cap;
+    k_histogram<KeyT><<<hist_blocks, HIST_THREADS, 0, s>>>(keys, n, passes, ctl);
+    k_scan_hist<<<passes, RADIX, 0, s>>>(ctl, status, status_stride);
+    const size_t dyn = (sizeof(KeyT) + sizeof(uint32_t)) * SORT_TILE;
+    static bool attr_done = false;
+    if (!attr_done) {
+        HCC_CUDA_TRY(cudaFuncSetAttribute(k_onesweep<KeyT, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+        HCC_CUDA_TRY(cudaFuncSetAttribute(k_onesweep<KeyT, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+        HCC_CUDA_TRY(cudaFuncSetAttribute(k_onesweep<KeyT, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+        HCC_CUDA_TRY(cudaFuncSetAttribute(k_onesweep<KeyT, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+        attr_done = true;
+    }
+    KeyT *kin = keys, *kout = keys_tmp;
+    for (uint32_t p = 0; p < passes; ++p) {
+        const bool first = p == 0, last = p + 1 == passes;
+        // the last pass must land in perm; value buffers alternate backwards from there
+        uint32_t *vout = ((passes - 1 - p) & 1u) ? vals_tmp : perm;
+        uint32_t *vin = ((passes - 1 - p) & 1u) ? perm : vals_tmp;
+        uint32_t *st = status + (size_t)p * status_stride;
+        uint32_t *tk = &ctl->ticket[p];
+        const uint32_t shift = RADIX_BITS * p;
+        if (first && last) k_onesweep<KeyT, true, false><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk);
+        else if (first)    k_onesweep<KeyT, true, true><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk);
+        else if (last)     k_onesweep<KeyT, false, false><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk);
+        else               k_onesweep<KeyT, false, true><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk);
+        KeyT *t = kin; kin = kout; kout = t;
+    }
+    HCC_CUDA_TRY(cudaGetLastError());
+    return HCC_OK;
+}
+
+}  // namespace hcc
+
+using namespace hcc;
+
+extern "C" int32_t hcc_sort_workspace_bytes(uint64_t n, uint32_t container_bits, uint64_t *bytes) {
+    HCC_REQUIRE(bytes, HCC_ERR_INVALID_ARG, "hcc_sort_workspace_bytes: NULL bytes");
+    HCC_REQUIRE(container_bits == 32 || container_bits == 64, HCC_ERR_INVALID_ARG, "hcc_sort: container_bits must be 32 or 64");
+    HCC_REQUIRE(n < (1ull << 30), HCC_ERR_UNSUPPORTED, "hcc_sort: n >= 2^30");
+    *bytes = round_up((container_bits / 8) * n, 256) + round_up(4 * n, 256) + ctl_bytes(n) + 256;
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_sort(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bits_used, uint32_t *perm_dev,
+                            void *workspace_dev, uint64_t workspace_bytes, void *stream) {
+    HCC_REQUIRE(container_bits == 32 || container_bits == 64, HCC_ERR_INVALID_ARG, "hcc_sort: container_bits must be 32 or 64");
+    HCC_REQUIRE(bits_used <= container_bits, HCC_ERR_INVALID_ARG, "hcc_sort: bits_used > container_bits");
+    HCC_REQUIRE(n < (1ull << 30), HCC_ERR_UNSUPPORTED, "hcc_sort: n >= 2^30");
+    if (n == 0) return HCC_OK;
+    HCC_REQUIRE(keys_dev && perm_dev && workspace_dev, HCC_ERR_INVALID_ARG, "hcc_sort: NULL argument");
+    HCC_REQUIRE(aligned(keys_dev, 16) && aligned(perm_dev, 16) && aligned(workspace_dev, 16), HCC_ERR_BAD_ALIGNMENT,
+                "hcc_sort: keys, perm and workspace need 16-byte alignment");
+    uint64_t need = 0;
+    hcc_sort_workspace_bytes(n, container_bits, &need);
+    HCC_REQUIRE(workspace_bytes >= need, HCC_ERR_INVALID_ARG, "hcc_sort: workspace too small (%llu < %llu)",
+                (unsigned long long)workspace_bytes, (unsigned long long)need);
+    cudaStream_t s = (cudaStream_t)stream;
+    const uint32_t passes = (bits_used + RADIX_BITS - 1) / RADIX_BITS;
+    if (passes == 0) {
+        k_iota<<<(uint32_t)((n + 255) / 256), 256, 0, s>>>(perm_dev, (uint32_t)n);
+        HCC_CUDA_TRY(cudaGetLastError());
+        return HCC_OK;
+    }
+    unsigned char *ws = reinterpret_cast<unsigned char *>(round_up(reinterpret_cast<uintptr_t>(workspace_dev), 256));
+    if (container_bits == 32) return sort_impl<uint32_t>((uint32_t *)keys_dev, (uint32_t)n, passes, perm_dev, ws, s);
+    return sort_impl<unsigned long long>((unsigned long long *)keys_dev, (uint32_t)n, passes, perm_dev, ws, s);
+}

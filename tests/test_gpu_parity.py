@@ -1,0 +1,374 @@
+"""Parity of the CUDA path (through the C ABI, via the thin binding) against the oracle, on
+the same seeded inputs.  Bars (BASELINE.json north_star): cut node sets, keys and the
+stable-sorted permutation bit-exact; hit prim ids identical wherever the two nearest
+candidate t differ by more than 1e-5 relative; hit t within 1e-5 relative; any-hit bits
+identical."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+REL_T = 1e-5
+
+
+@pytest.fixture(scope="module")
+def hcc():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2305_16652_b200 as h
+    return h
+
+
+@pytest.fixture(scope="module")
+def dev_cases(hcc, tiny, room_small, room_mid):
+    out = {}
+    for name, case in (("tiny", tiny), ("room_small", room_small), ("room_mid", room_mid)):
+        b = case.bvh
+        out[name] = dict(case=case, bvh=hcc.Bvh(b.nodes, b.tris, b.prim_idx),
+                         diffuse=torch.from_numpy(case.diffuse).cuda(),
+                         shadow=torch.from_numpy(case.shadow).cuda())
+    return out
+
+
+def _u32(t):
+    return t.detach().cpu().numpy().view(np.uint32)
+
+
+# ------------------------------------------------------------------------------- (a1)
+@pytest.mark.parametrize("name", ["tiny", "room_small"])
+@pytest.mark.parametrize("lam", [0.125, 0.3, 1.0])
+def test_density_bit_exact(hcc, dev_cases, name, lam):
+    import oracle
+    d = dev_cases[name]
+    got = hcc.density(d["bvh"], lam).cpu().numpy()
+    want = oracle.had(d["case"].bvh.nodes, lam)
+    assert np.array_equal(got.view(np.uint32), want.view(np.uint32))
+
+
+def test_bvh_info(hcc, dev_cases):
+    for d in dev_cases.values():
+        b = d["case"].bvh
+        assert d["bvh"].n_nodes == b.n_nodes and d["bvh"].n_tris == b.n_tris
+        assert d["bvh"].n_leaves == b.n_leaves and d["bvh"].max_depth == b.max_depth
+        assert np.array_equal(d["bvh"].scene_lo, b.nodes["lo"][0]) and np.array_equal(d["bvh"].scene_hi, b.nodes["hi"][0])
+
+
+CUT_REQUESTS = [(1, 32), (2, 16), (16, 16), (32, 32), (64, 64), (64, 32), (64, 16), (256, 32), (256, 16),
+                (1024, 32), (1024, 64), (4096, 64), (4096, 24), (16384, 64), (65536, 64), (65536, 32),
+                (48, 48), (100, 32), (1000, 48)]
+
+
+@pytest.mark.parametrize("name", ["tiny", "room_small"])
+@pytest.mark.parametrize("K,bits", CUT_REQUESTS)
+def test_select_cut_tables_bit_exact(hcc, dev_cases, name, K, bits):
+    import oracle
+    d = dev_cases[name]
+    nodes = d["case"].bvh.nodes
+    had = hcc.density(d["bvh"])
+    cut = hcc.select_cut(d["bvh"], had, K, bits)
+    info = cut.info()
+    tables, k_eff, _ = oracle.select_cut(nodes, K, bits)
+    assert info["widths"] == tables.widths and info["K_eff"] == k_eff
+    assert info["bits_used"] == tables.bits_used and info["container_bits"] == (32 if bits <= 32 else 64)
+    ent, cnt = cut.read()
+    assert np.array_equal(cnt, tables.table_cnt)
+    assert np.array_equal(ent, tables.entry_node)
+    cut.close()
+
+
+@pytest.mark.parametrize("widths,bits", [([8, 8], 16), ([16, 16], 32), ([32, 32], 64), ([4, 4, 4, 4], 16),
+                                         ([64], 64), ([3, 5, 7], 16), ([16, 8, 8], 32), ([1, 1, 2], 16)])
+def test_select_cut_levels_bit_exact(hcc, dev_cases, widths, bits):
+    import oracle
+    d = dev_cases["room_small"]
+    nodes = d["case"].bvh.nodes
+    had = hcc.density(d["bvh"])
+    cut = hcc.select_cut_levels(d["bvh"], had, widths, bits)
+    tables = oracle.level_tables(nodes, oracle.had(nodes), widths)
+    ent, cnt = cut.read()
+    assert np.array_equal(cnt, tables.table_cnt) and np.array_equal(ent, tables.entry_node)
+
+
+@pytest.mark.parametrize("name", ["tiny", "room_small"])
+def test_select_cut_flat_any_K(hcc, dev_cases, name):
+    import oracle
+    d = dev_cases[name]
+    nodes = d["case"].bvh.nodes
+    had_o = oracle.had(nodes)
+    had = hcc.density(d["bvh"])
+    n_leaves = d["case"].bvh.n_leaves
+    for K in [1, 2, 3, 7, 64, 65, 1000, 4096, 5000, n_leaves - 1, n_leaves, n_leaves + 5]:
+        out, cnt = hcc.select_cut_flat(d["bvh"], had, K)
+        c = int(cnt.cpu()[0])
+        want = oracle.cut(nodes, had_o, K)
+        assert c == want.shape[0] == min(K, n_leaves)
+        assert np.array_equal(_u32(out)[:c], want), K
+
+
+# ------------------------------------------------------------------------------- (a2)
+ENC_REQUESTS = [(64, 32), (32, 32), (64, 64), (1024, 32), (4096, 64), (16384, 64), (256, 16), (48, 48), (1000, 48)]
+
+
+@pytest.mark.parametrize("name", ["tiny", "room_mid"])
+@pytest.mark.parametrize("K,bits", ENC_REQUESTS)
+def test_encode_keys_bit_exact(hcc, dev_cases, name, K, bits):
+    import oracle
+    d = dev_cases[name]
+    nodes = d["case"].bvh.nodes
+    tables, _, _ = oracle.select_cut(nodes, K, bits)
+    cut = hcc.select_cut(d["bvh"], hcc.density(d["bvh"]), K, bits)
+    for batch in ("diffuse", "shadow"):
+        got = hcc.keys_to_numpy(hcc.encode(d[batch], cut))
+        want = oracle.encode_hcc(getattr(d["case"], batch), nodes, tables)
+        assert np.array_equal(got, want), (batch, int((got != want).sum()))
+        assert int(got.max()) < (1 << tables.bits_used)
+
+
+def test_encode_degenerate_rays(hcc, dev_cases):
+    """Axis-parallel directions (0 components), origins on box planes, rays missing the scene."""
+    import oracle
+    d = dev_cases["room_small"]
+    nodes = d["case"].bvh.nodes
+    rng = np.random.default_rng(5)
+    n = 5000
+    rays = np.zeros((n, 8), np.float32)
+    rays[:, 0:3] = rng.uniform(-0.5, 1.5, (n, 3))
+    dirs = rng.normal(size=(n, 3))
+    dirs[rng.uniform(size=(n, 3)) < 0.4] = 0.0
+    dirs[np.abs(dirs).sum(1) == 0, 0] = 1.0
+    dirs[rng.uniform(size=(n, 3)) < 0.1] *= -0.0
+    rays[:, 4:7] = dirs / np.linalg.norm(dirs, axis=1, keepdims=True)
+    rays[:, 7] = np.where(rng.uniform(size=n) < 0.5, np.inf, rng.uniform(0.01, 2.0, n))
+    # origins snapped onto cut-box planes
+    tables, _, _ = oracle.select_cut(nodes, 1024, 32)
+    boxes = nodes[tables.level_entries(0)[: tables.table_cnt[0]]]
+    for i in range(0, n, 7):
+        b = boxes[i % boxes.shape[0]]
+        a = i % 3
+        rays[i, a] = b["lo"][a] if (i // 3) % 2 else b["hi"][a]
+    cut = hcc.select_cut(d["bvh"], hcc.density(d["bvh"]), 1024, 32)
+    got = hcc.keys_to_numpy(hcc.encode(torch.from_numpy(rays).cuda(), cut))
+    want = oracle.encode_hcc(rays, nodes, tables)
+    assert np.array_equal(got, want)
+
+
+@pytest.mark.parametrize("bits", [16, 24, 32, 48, 64])
+def test_twopoint_keys_bit_exact(hcc, dev_cases, bits):
+    import oracle
+    for name in ("tiny", "room_mid"):
+        d = dev_cases[name]
+        lo, hi = d["bvh"].scene_lo, d["bvh"].scene_hi
+        for batch in ("diffuse", "shadow"):
+            got = hcc.keys_to_numpy(hcc.encode_twopoint(d[batch], lo, hi, bits))
+            want = oracle.encode_twopoint(getattr(d["case"], batch), lo, hi, bits)
+            assert np.array_equal(got, want)
+
+
+# ------------------------------------------------------------------------------- (a3)
+@pytest.mark.parametrize("cb", [32, 64])
+@pytest.mark.parametrize("n", [1, 2, 31, 33, 4095, 4096, 4097, 8192 + 5, 100003, 1 << 20])
+def test_sort_random_keys(hcc, cb, n):
+    import oracle
+    rng = np.random.default_rng(n * 3 + cb)
+    for bits_used in ([5, 8, 16, 20, 32] if cb == 32 else [9, 32, 40, 48, 64]):
+        if n > 200000 and bits_used not in (32, 48):
+            continue
+        hi = (1 << bits_used) - 1
+        keys = rng.integers(0, hi, size=n, dtype=np.uint64, endpoint=True)
+        if bits_used >= 16:         # long runs of equal keys exercise stability
+            keys[rng.uniform(size=n) < 0.3] = keys[0]
+        dt = np.uint32 if cb == 32 else np.uint64
+        kd = torch.from_numpy(keys.astype(dt).view(np.int32 if cb == 32 else np.int64)).cuda()
+        perm = _u32(hcc.sort(kd, bits_used))
+        assert np.array_equal(perm, oracle.sort(keys)), (n, cb, bits_used)
+
+
+def test_sort_zero_bits_and_empty(hcc):
+    kd = torch.zeros(1000, dtype=torch.int32, device="cuda")
+    assert np.array_equal(_u32(hcc.sort(kd, 0)), np.arange(1000, dtype=np.uint32))
+    e = torch.zeros(0, dtype=torch.int32, device="cuda")
+    assert hcc.sort(e, 32).shape[0] == 0
+
+
+@pytest.mark.parametrize("name,K,bits", [("tiny", 64, 32), ("room_mid", 1024, 32), ("room_mid", 4096, 64)])
+def test_sort_of_encoded_keys(hcc, dev_cases, name, K, bits):
+    import oracle
+    d = dev_cases[name]
+    cut = hcc.select_cut(d["bvh"], hcc.density(d["bvh"]), K, bits)
+    for batch in ("diffuse", "shadow"):
+        keys = hcc.encode(d[batch], cut)
+        k_host = hcc.keys_to_numpy(keys)
+        perm = _u32(hcc.sort(keys, cut.info()["bits_used"]))
+        assert np.array_equal(perm, oracle.sort(k_host))
+
+
+# ------------------------------------------------------------------------------- (a4)
+def _second_nearest_gap_ok(case, rays, idx, t_first):
+    """For the rays `idx` where prim ids differ: True where the two nearest candidate t are
+    within REL_T relative of each other (then either prim is a correct answer)."""
+    import oracle
+    ok = np.zeros(idx.shape[0], dtype=bool)
+    tris = case.bvh.tris.reshape(-1, 9)
+    for j, i in enumerate(idx):
+        ts = []
+        for k in range(tris.shape[0]):
+            hit, tuv = oracle.tri_hit(rays[i], tris[k])
+            if hit:
+                ts.append(float(tuv[0]))
+        ts.sort()
+        ok[j] = len(ts) >= 2 and (ts[1] - ts[0]) <= REL_T * abs(ts[0])
+    return ok
+
+
+def check_closest(case, rays, got, want):
+    gt, gp, gu, gv = got
+    wt, wp, wu, wv = want
+    assert np.array_equal(np.isinf(gt), np.isinf(wt)), "hit / miss sets differ"
+    hit = ~np.isinf(wt)
+    assert np.all(gp[~hit] == 0xFFFFFFFF)
+    rel = np.abs(gt[hit] - wt[hit]) / np.abs(wt[hit])
+    assert rel.size == 0 or rel.max() <= REL_T, rel.max()
+    diff = np.nonzero(gp != wp)[0]
+    assert diff.shape[0] <= 64, f"{diff.shape[0]} prim ids differ"
+    if diff.shape[0]:
+        assert _second_nearest_gap_ok(case, rays, diff, wt).all()
+    same = hit & (gp == wp)
+    assert np.allclose(gu[same], wu[same], rtol=0, atol=1e-4) and np.allclose(gv[same], wv[same], rtol=0, atol=1e-4)
+
+
+@pytest.mark.parametrize("name", ["tiny", "room_small", "room_mid"])
+def test_trace_closest_vs_oracle(hcc, dev_cases, name):
+    import oracle
+    d = dev_cases[name]
+    b = d["case"].bvh
+    want = oracle.closest_bvh(d["case"].diffuse, b.nodes, b.prim_idx, b.tris)
+    got = hcc.hits_to_numpy(hcc.trace(d["bvh"], d["diffuse"], None, hcc.TRACE_CLOSEST))
+    check_closest(d["case"], d["case"].diffuse, got, want)
+
+
+@pytest.mark.parametrize("name", ["tiny", "room_small", "room_mid"])
+def test_trace_any_vs_oracle(hcc, dev_cases, name):
+    import oracle
+    d = dev_cases[name]
+    b = d["case"].bvh
+    want = oracle.any_bvh(d["case"].shadow, b.nodes, b.prim_idx, b.tris)
+    got = hcc.trace(d["bvh"], d["shadow"], None, hcc.TRACE_ANY).cpu().numpy()
+    assert np.array_equal(got, want)
+    assert 0 < int(want.sum()) < want.shape[0]
+
+
+def test_trace_tiny_vs_brute_force(hcc, dev_cases):
+    """Config 1: the definition itself (all-triangle intersection)."""
+    import oracle
+    d = dev_cases["tiny"]
+    case = d["case"]
+    want = oracle.closest_brute(case.diffuse, case.bvh.tris)
+    got = hcc.hits_to_numpy(hcc.trace(d["bvh"], d["diffuse"], None, hcc.TRACE_CLOSEST))
+    check_closest(case, case.diffuse, got, want)
+    occ = hcc.trace(d["bvh"], d["shadow"], None, hcc.TRACE_ANY).cpu().numpy()
+    assert np.array_equal(occ, oracle.any_brute(case.shadow, case.bvh.tris))
+
+
+def test_trace_primary_rays_with_misses(hcc, dev_cases):
+    import oracle
+    d = dev_cases["tiny"]
+    case = d["case"]
+    prim = case.w.primaries()
+    want = oracle.closest_bvh(prim, case.bvh.nodes, case.bvh.prim_idx, case.bvh.tris)
+    got = hcc.hits_to_numpy(hcc.trace(d["bvh"], torch.from_numpy(prim).cuda(), None, hcc.TRACE_CLOSEST))
+    assert np.isinf(want[0]).any() and (~np.isinf(want[0])).any()
+    check_closest(case, prim, got, want)
+
+
+@pytest.mark.parametrize("name,K,bits", [("tiny", 64, 32), ("room_mid", 1024, 32)])
+def test_trace_through_perm_writes_by_ray_id(hcc, dev_cases, name, K, bits):
+    """Thread j traces ray perm[j]; results land at the ray's own index, so the
+    reordered results are bit-identical to the NoSort ones."""
+    d = dev_cases[name]
+    cut = hcc.select_cut(d["bvh"], hcc.density(d["bvh"]), K, bits)
+    for batch, mode in (("diffuse", hcc.TRACE_CLOSEST), ("shadow", hcc.TRACE_ANY)):
+        perm = hcc.sort(hcc.encode(d[batch], cut), cut.info()["bits_used"])
+        a = hcc.trace(d["bvh"], d[batch], None, mode)
+        b = hcc.trace(d["bvh"], d[batch], perm, mode)
+        assert torch.equal(a.view(torch.uint8), b.view(torch.uint8))
+
+
+def test_trace_stats_and_anc(hcc, dev_cases):
+    import oracle
+    d = dev_cases["room_small"]
+    b = d["case"].bvh
+    st = hcc.trace_stats(d["bvh"], d["diffuse"], None, hcc.TRACE_CLOSEST)
+    assert st["rays"] == d["diffuse"].shape[0] and st["pairs"] > 0 and st["tris"] > 0
+    assert st["max_stack"] <= b.max_depth
+    cut = hcc.select_cut(d["bvh"], hcc.density(d["bvh"]), 1024, 32)
+    keys = hcc.encode(d["diffuse"], cut)
+    k_host = hcc.keys_to_numpy(keys)
+    kept = keys.clone()
+    perm = hcc.sort(keys, cut.info()["bits_used"])
+    for p_dev, p_host in ((None, np.arange(k_host.shape[0])), (perm, _u32(perm))):
+        ks = k_host[p_host]
+        n_w = (ks.shape[0] + 31) // 32
+        want = sum(len(np.unique(ks[32 * w:32 * w + 32])) for w in range(n_w)) / n_w
+        assert abs(hcc.anc(kept, p_dev) - want) < 1e-9
+
+
+# ------------------------------------------------------------------------------- pipeline
+@pytest.mark.parametrize("name,K,bits", [("tiny", 64, 32), ("room_mid", 1024, 32), ("room_mid", 4096, 64)])
+def test_pipeline_matches_stages(hcc, dev_cases, name, K, bits):
+    import oracle
+    d = dev_cases[name]
+    case = d["case"]
+    cut = hcc.select_cut(d["bvh"], hcc.density(d["bvh"]), K, bits)
+    n_max = max(d["diffuse"].shape[0], d["shadow"].shape[0])
+    pipe = hcc.Pipeline(n_max, 64, host_staging=True)
+    for batch, mode in (("diffuse", hcc.TRACE_CLOSEST), ("shadow", hcc.TRACE_ANY)):
+        ref = hcc.trace(d["bvh"], d[batch], None, mode)
+        for order in (hcc.ORDER_NOSORT, hcc.ORDER_TWOPOINT, hcc.ORDER_HCC):
+            perm_out = torch.full((d[batch].shape[0],), -1, dtype=torch.int32, device="cuda")
+            got = pipe.reorder_trace(d["bvh"], cut, order, d[batch], mode, key_bits=bits, perm_out=perm_out)
+            assert torch.equal(got.view(torch.uint8), ref.view(torch.uint8))
+            ms = pipe.stage_ms()
+            assert ms["trace"] > 0
+            if order == hcc.ORDER_HCC:
+                tables, _, _ = oracle.select_cut(case.bvh.nodes, K, bits)
+                want = oracle.sort(oracle.encode_hcc(getattr(case, batch), case.bvh.nodes, tables))
+                assert np.array_equal(_u32(perm_out), want)
+            # host-buffer form
+            rays_h = torch.from_numpy(getattr(case, batch)).pin_memory()
+            hits_h = torch.empty(ref.shape, dtype=ref.dtype).pin_memory()
+            pipe.reorder_trace_host(d["bvh"], cut, order, rays_h, hits_h, mode, key_bits=bits)
+            assert torch.equal(hits_h.view(torch.uint8), ref.cpu().view(torch.uint8))
+    pipe.close()
+
+
+# ------------------------------------------------------------------------------- errors
+def test_error_reporting(hcc, dev_cases):
+    d = dev_cases["tiny"]
+    had = hcc.density(d["bvh"])
+    with pytest.raises(hcc.HccError) as e:
+        hcc.select_cut(d["bvh"], had, 0, 32)
+    assert e.value.status == -1 and "K" in str(e.value)
+    with pytest.raises(hcc.HccError):
+        hcc.select_cut(d["bvh"], had, 64, 20)
+    cut = hcc.Cut(64)
+    with pytest.raises(hcc.HccError):
+        hcc.encode(d["diffuse"], cut)            # no selection yet
+    keys = torch.zeros(9, dtype=torch.int32, device="cuda")
+    with pytest.raises(hcc.HccError) as e:
+        hcc.sort(keys[1:], 32)                    # 4-byte offset: misaligned
+    assert e.value.status == -2
+    with pytest.raises(hcc.HccError):
+        hcc.sort(torch.zeros(8, dtype=torch.int32, device="cuda"), 40)
+    with pytest.raises(hcc.HccError):
+        hcc.trace(d["bvh"], d["diffuse"], None, 7)
+    bad = d["case"].bvh.nodes.copy()
+    bad["left_or_first"][0] = 0                   # child not after its parent
+    with pytest.raises(hcc.HccError):
+        hcc.Bvh(bad, d["case"].bvh.tris, d["case"].bvh.prim_idx)
+    # n = 0 is a no-op everywhere
+    empty = torch.zeros((0, 8), dtype=torch.float32, device="cuda")
+    cut = hcc.select_cut(d["bvh"], had, 64, 32)
+    assert hcc.encode(empty, cut).shape[0] == 0
+    assert hcc.trace(d["bvh"], empty, None, hcc.TRACE_ANY).shape[0] == 0
