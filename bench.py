@@ -1,0 +1,440 @@
+"""bench.py — the hot path of hierarchy-cut-code ray reordering on B200, measured.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload room|fig1|tiny]
+
+One STEP = one pass of the whole per-batch hot path (Figure 11) over one
+bounce of BASELINE.json config 2 ("room": 64,012 triangles, 512x512x4 spp): the diffuse batch
+(1,048,576 closest-hit rays) and the shadow batch (2,097,152 any-hit rays), each
+key-computed (hcc_encode), sorted (hcc_sort) and traced through the sorted indices (hcc_trace)
+in ONE C-ABI call, hcc_reorder_trace.  Metric: secondary Mrays/s INCLUDING encode + sort.
+The same rays are also run in the NoSort and TwoPoint orders and the
+per-stage split, speed-ups, ANC and roofline fractions are reported in the
+JSON line.  The cut (hcc_density + hcc_select_cut) is a once-per-scene pre-process in the
+paper (:157, :218); it is timed separately ("cut_ms").
+
+Inputs are seeded and synthetic (hcc_inputs/); the primaries are
+traced by the library's own tracer (parity-tested against the oracle in tests/).  L2 is
+flushed between timed steps (the batches, 100 MB, would otherwise sit in the 126 MB L2).
+
+--impl reference times the CPU oracle (oracle/, single-threaded C) on a bounded sample of the
+same workload; it is the only mode, with the cpu_baseline leg, that touches oracle/.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "secondary Mrays/s incl. encode+sort (hierarchy cut code order; diffuse + shadow batches of one bounce)"
+UNIT = "Mrays/s"
+
+# Algorithmic work per ray, stated in DESIGN.md "Rooflines":
+#  encode: 32 B ray read + key write;  sort: one histogram read + per pass read+write of (key, id)
+#  trace : fp32 lane-operations = 26 per box test + 36 per triangle test (operation counts of the
+#          formulas in include/hcc.h), box tests = 2 per sibling pair fetched.
+OPS_BOX, OPS_TRI = 26, 36
+SM_COUNT, LANES_PER_SM = 148, 128
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    except Exception:
+        return 6650.0, 1965.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc, self.thread = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ts, line in self.rows:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                c, m = float(f[0]), float(f[1])
+            except ValueError:
+                continue
+            smax = m
+            if t0 - 0.05 <= ts <= t1 + 0.15:
+                sm.append(c)
+                for nm, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+        if not sm:   # region shorter than a sample period: take whatever was seen
+            for ts, line in self.rows:
+                f = [x.strip() for x in line.split(",")]
+                try:
+                    sm.append(float(f[0]))
+                except Exception:
+                    pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------
+def _oracle_tracer():
+    import oracle
+
+    def trace_closest(bvh, rays):
+        t, p, _, _ = oracle.closest_bvh(rays, bvh.nodes, bvh.prim_idx, bvh.tris)
+        return t, p
+    return trace_closest
+
+
+def oracle_pass(w, diffuse, shadow):
+    """One pass of the hot path in the oracle: encode + stable sort + BVH traversal of both
+    batches.  Returns seconds per stage."""
+    import oracle
+    b = w.bvh
+    tables, _, _ = oracle.select_cut(b.nodes, w.K, w.key_bits)
+    out = {"encode": 0.0, "sort": 0.0, "trace": 0.0}
+    for rays, closest in ((diffuse, True), (shadow, False)):
+        t0 = time.perf_counter()
+        keys = oracle.encode_hcc(rays, b.nodes, tables)
+        t1 = time.perf_counter()
+        perm = oracle.sort(keys)
+        t2 = time.perf_counter()
+        r = np.ascontiguousarray(rays[perm])    # "fetches the rays based on these sorted indices"
+        if closest:
+            oracle.closest_bvh(r, b.nodes, b.prim_idx, b.tris)
+        else:
+            oracle.any_bvh(r, b.nodes, b.prim_idx, b.tris)
+        t3 = time.perf_counter()
+        out["encode"] += t1 - t0; out["sort"] += t2 - t1; out["trace"] += t3 - t2
+    return out
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands, single-threaded, on a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import hcc_inputs
+    w = hcc_inputs.Workload(args.workload)
+    n_d = min(args.ref_sample, w.width * w.height * w.spp)
+    prim = w.primaries()[:n_d]
+    t, p = _oracle_tracer()(w.bvh, prim)
+    diffuse, shadow, _ = w.bounce(1, prim, t, p)
+    n = diffuse.shape[0] + shadow.shape[0]
+    for _ in range(args.warmup):
+        oracle_pass(w, diffuse, shadow)
+    t0 = time.perf_counter()
+    split = {"encode": 0.0, "sort": 0.0, "trace": 0.0}
+    for _ in range(args.steps):
+        s = oracle_pass(w, diffuse, shadow)
+        for k in split:
+            split[k] += s[k]
+    dt = time.perf_counter() - t0
+    val = n * args.steps / dt / 1e6
+    sample = (f"first {diffuse.shape[0]} diffuse + {shadow.shape[0]} shadow rays of the bounce "
+              f"(primary-sample order) per step")
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic", "config": _config(args, w, diffuse.shape[0], shadow.shape[0], l2="n/a (CPU)"),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                             "split_s": {k: v / args.steps for k, v in split.items()}, "host_cores": os.cpu_count()},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def _config(args, w, n_d, n_s, l2):
+    return {"workload": f"config 2 'room' of BASELINE.json" if args.workload == "room" else args.workload,
+            "triangles": int(w.bvh.n_tris), "bvh_nodes": int(w.bvh.n_nodes), "K": int(w.K),
+            "key_bits": int(w.key_bits), "diffuse_rays": int(n_d), "shadow_rays": int(n_s),
+            "resolution": f"{w.width}x{w.height}x{w.spp}spp", "bounce": 1, "l2": l2,
+            "parallelism": f"rays sharded over {args.gpus} GPU(s), BVH and cut replicated, no collective"}
+
+
+# ------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import hcc_inputs
+    from paper_2305_16652_b200 import build as cuda_build
+    cuda_build.build()
+    import paper_2305_16652_b200 as hcc
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    hbm_gbs, sm_max_mhz, peak_kind = _peaks()
+
+    # ---- inputs (seeded; rank r draws its own sub-pixel samples of the same scene)
+    w = hcc_inputs.Workload(args.workload, rank=rank)
+    b = w.bvh
+    bvh = hcc.Bvh(b.nodes, b.tris, b.prim_idx)
+
+    def gpu_trace_closest(_bvh, rays):
+        h = hcc.trace(bvh, torch.from_numpy(rays).cuda(), None, hcc.TRACE_CLOSEST)
+        t, p, _, _ = hcc.hits_to_numpy(h)
+        return t, p
+    diffuse_h, shadow_h = w.first_bounce(gpu_trace_closest)
+    n_d, n_s = diffuse_h.shape[0], shadow_h.shape[0]
+    n = n_d + n_s
+    diffuse = torch.from_numpy(diffuse_h).cuda()
+    shadow = torch.from_numpy(shadow_h).cuda()
+    batches = ((diffuse, hcc.TRACE_CLOSEST, "diffuse"), (shadow, hcc.TRACE_ANY, "shadow"))
+
+    # ---- pre-process (once per scene): density + cut
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    had = hcc.density(bvh)
+    cut = hcc.select_cut(bvh, had, w.K, w.key_bits)
+    torch.cuda.synchronize()
+    e0, e1 = ev(), ev()
+    e0.record()
+    hcc.density(bvh, out=had)
+    hcc.select_cut(bvh, had, w.K, w.key_bits, cut=cut)
+    e1.record()
+    torch.cuda.synchronize()
+    cut_ms = e0.elapsed_time(e1)
+    info = cut.info()
+    container = info["container_bits"]
+    passes = (info["bits_used"] + 7) // 8
+
+    pipe = hcc.Pipeline(max(n_d, n_s), 64, host_staging=True)
+    hits_d = torch.empty((n_d, 4), dtype=torch.float32, device="cuda")
+    hits_s = torch.empty(n_s, dtype=torch.uint8, device="cuda")
+    hits = {"diffuse": hits_d, "shadow": hits_s}
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.int32, device="cuda")   # 256 MiB > 126 MB L2
+
+    def step(order):
+        for rays, mode, name in batches:
+            pipe.reorder_trace(bvh, cut, order, rays, mode, hits=hits[name], key_bits=w.key_bits)
+
+    def timed(order, steps, warmup, per_stage=False):
+        for _ in range(warmup):
+            step(order)
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        pairs = [(ev(), ev()) for _ in range(steps)]
+        stage = {nm: {"encode": 0.0, "sort": 0.0, "trace": 0.0} for _, _, nm in batches}
+        t0 = time.time()
+        for s, e in pairs:
+            flush.zero_()                       # L2 flush, outside the event bracket
+            s.record()
+            if per_stage:
+                for rays, mode, name in batches:
+                    pipe.reorder_trace(bvh, cut, order, rays, mode, hits=hits[name], key_bits=w.key_bits)
+                    ms = pipe.stage_ms()
+                    for k in stage[name]:
+                        stage[name][k] += ms[k] / steps
+            else:
+                step(order)
+            e.record()
+        torch.cuda.synchronize()
+        t1 = time.time()
+        if world > 1:
+            dist.barrier()
+        ms = sum(s.elapsed_time(e) for s, e in pairs)
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms / steps, stage, (t0, t1)
+
+    # ---- the timed region: K steps of the HCC-ordered hot path
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    ms_step, _, (t0, t1) = timed(hcc.ORDER_HCC, args.steps, args.warmup)
+    clocks = sampler.stop(t0, t1) if rank == 0 else None
+    value = world * n / (ms_step * 1e-3) / 1e6
+
+    # ---- stage split and the comparison orders on the same rays (short runs, same hygiene)
+    k_cmp = max(3, min(args.steps, 10))
+    orders = {}
+    for name, order in (("hcc", hcc.ORDER_HCC), ("twopoint", hcc.ORDER_TWOPOINT), ("nosort", hcc.ORDER_NOSORT)):
+        ms, stage, _ = timed(order, k_cmp, 3, per_stage=True)
+        o = {"ms_per_step": ms, "mrays_per_s_incl": n / ms / 1e3}
+        for bn, nb in (("diffuse", n_d), ("shadow", n_s)):
+            st = stage[bn]
+            tot = st["encode"] + st["sort"] + st["trace"]
+            o[bn] = {"encode_ms": st["encode"], "sort_ms": st["sort"], "trace_ms": st["trace"],
+                     "mrays_per_s_incl": nb / tot / 1e3, "mrays_per_s_trace_only": nb / st["trace"] / 1e3}
+        orders[name] = o
+    speed = {}
+    for bn in ("diffuse", "shadow"):
+        h = orders["hcc"][bn]
+        speed[bn] = {"incl_vs_nosort": h["mrays_per_s_incl"] / orders["nosort"][bn]["mrays_per_s_incl"],
+                     "incl_vs_twopoint": h["mrays_per_s_incl"] / orders["twopoint"][bn]["mrays_per_s_incl"],
+                     "trace_vs_nosort": h["mrays_per_s_trace_only"] / orders["nosort"][bn]["mrays_per_s_trace_only"],
+                     "trace_vs_twopoint": h["mrays_per_s_trace_only"] / orders["twopoint"][bn]["mrays_per_s_trace_only"]}
+    speed["all_incl_vs_nosort"] = orders["nosort"]["ms_per_step"] / orders["hcc"]["ms_per_step"]
+    speed["all_incl_vs_twopoint"] = orders["twopoint"]["ms_per_step"] / orders["hcc"]["ms_per_step"]
+
+    # ---- trace work counters (instrumented kernel, never timed) and ANC, HCC order
+    diag = {}
+    alu_peak = SM_COUNT * LANES_PER_SM * sm_max_mhz * 1e6 / 1e12     # T lane-op/s
+    for rays, mode, name in batches:
+        keys = hcc.encode(rays, cut)
+        keys0 = keys.clone()
+        perm = hcc.sort(keys, info["bits_used"])
+        st = hcc.trace_stats(bvh, rays, perm, mode)
+        st0 = hcc.trace_stats(bvh, rays, None, mode)
+        ops = (2 * st["pairs"] * OPS_BOX + st["tris"] * OPS_TRI)
+        diag[name] = {"anc_hcc": hcc.anc(keys0, perm), "anc_nosort": hcc.anc(keys0, None),
+                      "node_bytes_per_ray": st["node_bytes_per_ray"], "tri_bytes_per_ray": st["tri_bytes_per_ray"],
+                      "node_bytes_per_ray_nosort": st0["node_bytes_per_ray"], "max_stack": st["max_stack"],
+                      "lane_ops_per_ray": ops / rays.shape[0], "lane_ops": ops}
+    nrays = {"diffuse": n_d, "shadow": n_s}
+    key_b = container // 8
+    stages = {}
+    for name in ("diffuse", "shadow"):
+        o, nb = orders["hcc"][name], nrays[name]
+        enc_bytes = nb * (32 + key_b)
+        sort_bytes = nb * (key_b + passes * 2 * (key_b + 4))
+        enc_gbs = enc_bytes / (o["encode_ms"] * 1e-3) / 1e9
+        sort_gbs = sort_bytes / (o["sort_ms"] * 1e-3) / 1e9
+        tr = diag[name]["lane_ops"] / (o["trace_ms"] * 1e-3) / 1e12
+        enc_ops = nb * info["bits_used"] * OPS_BOX / (o["encode_ms"] * 1e-3) / 1e12
+        stages[name] = {
+            "encode": {"bound": "hbm", "achieved": enc_gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": enc_gbs / hbm_gbs,
+                       "alu_achieved_tlaneops": enc_ops, "alu_frac": enc_ops / alu_peak, "box_tests_per_ray": info["bits_used"]},
+            "sort": {"bound": "hbm", "achieved": sort_gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": sort_gbs / hbm_gbs,
+                     "passes": passes},
+            "trace": {"bound": "alu", "achieved": tr, "peak": alu_peak, "unit": "Tlaneop/s", "frac": tr / alu_peak}}
+    # dominant kernel of the step = the closest-hit traversal of the diffuse batch
+    dom = max((("diffuse", "trace"), ("shadow", "trace"), ("diffuse", "sort"), ("shadow", "sort"),
+               ("diffuse", "encode"), ("shadow", "encode")), key=lambda k: orders["hcc"][k[0]][k[1] + "_ms"])
+    roof = dict(stages[dom[0]][dom[1]])
+    roof = {"bound": roof["bound"], "achieved": roof["achieved"], "peak": roof["peak"], "unit": roof["unit"],
+            "frac": roof["frac"], "traffic": None, "kernel": f"{dom[1]} ({dom[0]} batch)",
+            "peak_source": (f"{peak_kind} HBM copy" if roof["bound"] == "hbm" else
+                            f"148 SMs x 128 fp32 lanes x {sm_max_mhz:.0f} MHz (DESIGN.md)")}
+
+    # ---- e2e: the same step through the C ABI with HOST buffers (pinned), copies inside the timing
+    rays_pin = {"diffuse": torch.from_numpy(diffuse_h).pin_memory(), "shadow": torch.from_numpy(shadow_h).pin_memory()}
+    hits_pin = {"diffuse": torch.empty((n_d, 4), dtype=torch.float32).pin_memory(),
+                "shadow": torch.empty(n_s, dtype=torch.uint8).pin_memory()}
+
+    def step_host():
+        for _, mode, name in batches:
+            pipe.reorder_trace_host(bvh, cut, hcc.ORDER_HCC, rays_pin[name], hits_pin[name], mode, key_bits=w.key_bits)
+    for _ in range(3):
+        step_host()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    k_e2e = max(3, min(args.steps, 10))
+    e2e_ms = 0.0
+    for _ in range(k_e2e):
+        flush.zero_()
+        s, e = ev(), ev()
+        s.record()
+        step_host()
+        e.record()
+        torch.cuda.synchronize()
+        e2e_ms += s.elapsed_time(e) / k_e2e
+    if world > 1:
+        t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    assert torch.equal(hits_pin["shadow"].cuda(), hits_s) and torch.equal(hits_pin["diffuse"].cuda().view(torch.int32), hits_d.view(torch.int32))
+    e2e = {"value": world * n / e2e_ms / 1e3, "unit": UNIT, "ms_per_step": e2e_ms,
+           "h2d_bytes_per_step": 32 * n, "d2h_bytes_per_step": 16 * n_d + n_s}
+
+    # kernels launched per step: per batch 1 key kernel + (histogram + scan + one per digit) + 1 trace
+    launches_per_step = 2 * (1 + (2 + passes) + 1)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- cpu_baseline: the oracle on this box's host cores, bounded sample, rank 0, N = 1 only
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        m_d = min(n_d, args.cpu_sample)
+        d_s, s_s = diffuse_h[:m_d], shadow_h[:2 * m_d]
+        t0 = time.perf_counter()
+        split = oracle_pass(w, d_s, s_s)
+        dt = time.perf_counter() - t0
+        cpu = {"value": (d_s.shape[0] + s_s.shape[0]) / dt / 1e6, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"first {d_s.shape[0]} diffuse + {s_s.shape[0]} shadow rays of the same batches, one pass "
+                         f"(encode + stable sort + BVH traversal), {dt:.1f} s",
+               "split_s": split, "host_cores": os.cpu_count()}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": _config(args, w, n_d, n_s, l2="flushed between timed steps (256 MiB write)"),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
+            "roofline": roof, "cpu_baseline": cpu,
+            "cut": {"widths": info["widths"], "K_eff": info["K_eff"], "bits_used": info["bits_used"],
+                    "container_bits": container, "cut_ms": cut_ms},
+            "orders": orders, "speedup_hcc": speed, "stages_roofline_hcc": stages, "diagnostics": diag,
+            "paper_context": "RTX 3060, Breakfast: HCC 67.6 vs NoSort 37.4 vs TwoPoint 56.8 Mrays/s trace-only (PAPER.md:294-299); not comparable"}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="room", choices=["tiny", "room", "fig1", "large"])
+    ap.add_argument("--cpu-sample", type=int, default=1 << 20, help="diffuse rays in the cpu_baseline sample")
+    ap.add_argument("--ref-sample", type=int, default=1 << 15, help="diffuse rays per step of --impl reference")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,75 @@
+"""Multi-GPU host logic on CPU (gloo, world_size 2): contiguous ray shards tile the batch, and
+per-shard results gathered in rank order equal the single-process result (rays are independent in
+encode and trace).  The per-shard compute here is the oracle (tests may use it)."""
+import os
+import socket
+
+import numpy as np
+import pytest
+
+
+def test_ray_shard_tiles_the_batch():
+    from paper_2305_16652_b200.shard import ray_shard
+    for n in (0, 1, 2, 7, 4096, 1048576 + 3):
+        for world in (1, 2, 3, 8):
+            spans = [ray_shard(n, r, world) for r in range(world)]
+            assert spans[0][0] == 0 and spans[-1][1] == n
+            assert all(a[1] == b[0] for a, b in zip(spans, spans[1:]))
+            sizes = [b - a for a, b in spans]
+            assert max(sizes) - min(sizes) <= 1
+    with pytest.raises(ValueError):
+        ray_shard(10, 2, 2)
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, rays, nodes, prim_idx, tris, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    import torch
+    import torch.distributed as dist
+    import oracle
+    from paper_2305_16652_b200.shard import gather_hits, ray_shard
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        a, b = ray_shard(rays.shape[0], rank, world)
+        mine = rays[a:b]
+        tables, _, _ = oracle.select_cut(nodes, 64, 32)
+        keys = oracle.encode_hcc(mine, nodes, tables)
+        perm = oracle.sort(keys)                       # coherence is created per shard
+        t, p, _, _ = oracle.closest_bvh(np.ascontiguousarray(mine[perm]), nodes, prim_idx, tris)
+        local = np.empty((b - a, 2), dtype=np.float64)
+        local[perm, 0] = t                             # results land at the ray's own index
+        local[perm, 1] = p
+        full = gather_hits(torch.from_numpy(local), rays.shape[0])
+        keys_full = gather_hits(torch.from_numpy(keys.astype(np.int64)), rays.shape[0])
+        if rank == 0:
+            out.put((full.numpy(), keys_full.numpy()))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_sharded_path_equals_single_process(tiny):
+    import torch.multiprocessing as mp
+    import oracle
+    rays = tiny.diffuse[:1001]                         # odd size: shards of 501 and 500
+    b = tiny.bvh
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, rays, b.nodes, b.prim_idx, b.tris, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    full, keys_full = q.get(timeout=120)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    t, prim, _, _ = oracle.closest_bvh(rays, b.nodes, b.prim_idx, b.tris)
+    tables, _, _ = oracle.select_cut(b.nodes, 64, 32)
+    assert np.array_equal(full[:, 0], t.astype(np.float64))
+    assert np.array_equal(full[:, 1], prim.astype(np.float64))
+    assert np.array_equal(keys_full.astype(np.uint64), oracle.encode_hcc(rays, b.nodes, tables))
