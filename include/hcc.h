@@ -98,9 +98,11 @@ HCC_API int32_t hcc_version(void);
  * hcc_bvh_create validates the canonical arrays on the host (indices in range, siblings
  * adjacent, parent < child, every node reachable once, leaf count in 1..8, depth <= 63:
  * otherwise HCC_ERR_INVALID_ARG / HCC_ERR_UNSUPPORTED), copies them to the device and runs
- * the conversion kernels on `stream`: the 32-byte traversal records (sibling pairs
- * contiguous and 64-byte aligned), the 48-byte triangle records in leaf order, parent
- * links and sub-tree leaf counts.  All three arrays are host pointers, read before return.
+ * the conversion kernels on `stream`: one 32-byte traversal record per internal node
+ * (both child boxes as 15-bit cells of a uniform grid over the root box, rounded outwards
+ * and padded by one cell, plus the two child references), the 64-byte triangle records in
+ * leaf order, parent links and sub-tree leaf counts.  The quantised boxes only cull: results
+ * are defined by the triangle predicate under hcc_trace.  All three arrays are host pointers, read before return.
  * The call synchronises `stream` before returning. */
 HCC_API int32_t hcc_bvh_create(const hcc_node *nodes_host, uint32_t n_nodes, const float *tris_host,
                        uint32_t n_tris, const uint32_t *prim_idx_host, void *stream,
@@ -195,8 +197,9 @@ HCC_API int32_t hcc_sort(void *keys_dev, uint64_t n, uint32_t container_bits, ui
                  uint32_t *perm_dev, void *workspace_dev, uint64_t workspace_bytes, void *stream);
 
 /* ---- (a4) trace -----------------------------------------------------------------------
- * Thread j traces ray perm_dev[j] (perm_dev == NULL: ray j, the NoSort order) and writes
- * the result at the ray's own index ("the trace kernel fetches the rays based
+ * Rays are traced in the order perm_dev[0], perm_dev[1], ... (perm_dev == NULL: 0, 1, ...,
+ * the NoSort order): warps take consecutive 32-rank chunks of that order, and every result
+ * is written at the ray's own index ("the trace kernel fetches the rays based
  * on these sorted indices").  CLOSEST: hits_dev = hcc_hit[n]: the triangle with the
  * smallest t in (tmin, tmax), ties to the lowest prim id.  ANY: hits_dev = uint8[n].
  * Triangle test (fp32, fmaf where written): e1 = v1-v0, e2 = v2-v0, p = d x e2,
@@ -207,8 +210,8 @@ HCC_API int32_t hcc_trace(const hcc_bvh *bvh, const float *rays_dev, uint64_t n,
                   int32_t mode, void *hits_dev, void *stream);
 
 /* Same traversal, instrumented (never used for timing): stats_dev = uint64[4], zeroed by the
- * call, then [0] = sibling pairs fetched (64 bytes each), [1] = triangle records fetched
- * (48 bytes each), [2] = rays traced, [3] = deepest traversal stack.  hits_dev as hcc_trace. */
+ * call, then [0] = sibling-pair records fetched (32 bytes each), [1] = triangle records fetched
+ * (64 bytes each), [2] = rays traced, [3] = deepest traversal stack.  hits_dev as hcc_trace. */
 HCC_API int32_t hcc_trace_stats(const hcc_bvh *bvh, const float *rays_dev, uint64_t n, const uint32_t *perm_dev,
                         int32_t mode, void *hits_dev, uint64_t *stats_dev, void *stream);
 

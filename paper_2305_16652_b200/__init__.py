@@ -305,7 +305,7 @@ def trace_stats(bvh, rays, perm=None, mode=TRACE_CLOSEST, stream=None):
                                  _vp(st.data_ptr()), _stream(stream)))
     pairs, tris, nr, depth = [int(x) for x in st.cpu().tolist()]
     return dict(pairs=pairs, tris=tris, rays=nr, max_stack=depth,
-                node_bytes_per_ray=64.0 * pairs / max(nr, 1), tri_bytes_per_ray=48.0 * tris / max(nr, 1))
+                node_bytes_per_ray=32.0 * pairs / max(nr, 1), tri_bytes_per_ray=64.0 * tris / max(nr, 1))
 
 
 def anc(keys, perm=None, stream=None):

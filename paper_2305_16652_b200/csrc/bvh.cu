@@ -23,34 +23,62 @@ void set_error(const char *fmt, ...) {
 // conversion kernels
 // ---------------------------------------------------------------------------------------
 
-// Traversal record of node i, stored at record index i+1 so that a sibling pair
-// (left odd in the canonical numbering) starts on a 64-byte boundary:
-//   rec[2*(i+1)+0] = (lo.x, lo.y, lo.z, ref)      rec[2*(i+1)+1] = (hi.x, hi.y, hi.z, 0)
-//   ref, internal: record index of the left child = left + 1   (bit 31 clear)
-//   ref, leaf    : 0x80000000 | (count-1) << 28 | first triangle slot
-__global__ void k_convert_nodes(const hcc_node *__restrict__ nodes, uint32_t n, float4 *__restrict__ rec,
-                                uint32_t *__restrict__ parent) {
+// Traversal records.  Nothing on the results depends on them: the hit a ray reports is defined
+// by the triangle predicate alone (include/hcc.h), box culling only has to be conservative.
+// So the child boxes are stored compactly: the k-th INTERNAL node (node order) owns one
+// 32-byte record holding BOTH children, fetched with one 256-bit load per traversal step:
+//   w[0..2] = left child x, y, z:  lo cell | hi cell << 16     w[3..5] = right child
+//   w[6], w[7] = left, right child reference
+//   reference, internal child: (rank of the child among internal nodes) + 1      (bit 31 clear)
+//   reference, leaf child    : 0x80000000 | (count-1) << 28 | first triangle slot
+// Cells are indices of a uniform grid over the root box, g = (x - q_lo) * q_scale + 2 in fp32
+// (a monotone map, so containment survives it), lo = floor(g) - 1, hi = ceil(g) + 1, clamped to
+// [0, 32767]: every stored box contains the fp32 box with a margin of at least one cell
+// (3e-5 of the scene extent), far above the rounding of the slab arithmetic in trace.cu.
+__global__ void k_parents(const hcc_node *__restrict__ nodes, uint32_t n, uint32_t *__restrict__ parent) {
     uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     hcc_node nd = nodes[i];
-    uint32_t ref;
     if (nd.count == 0) {
-        ref = nd.left_or_first + 1u;
         parent[nd.left_or_first] = i;
         parent[nd.left_or_first + 1u] = i;
-    } else {
-        ref = 0x80000000u | ((nd.count - 1u) << 28) | nd.left_or_first;
     }
     if (i == 0) parent[0] = 0xFFFFFFFFu;
-    rec[2 * (size_t)(i + 1) + 0] = make_float4(nd.lo[0], nd.lo[1], nd.lo[2], __uint_as_float(ref));
-    rec[2 * (size_t)(i + 1) + 1] = make_float4(nd.hi[0], nd.hi[1], nd.hi[2], 0.0f);
-    if (i == 0) {  // record 0 is padding
-        rec[0] = make_float4(0.f, 0.f, 0.f, 0.f);
-        rec[1] = make_float4(0.f, 0.f, 0.f, 0.f);
-    }
 }
 
-// Triangle record k (leaf order): (v0, prim id), (e1 = v1 - v0, 0), (e2 = v2 - v0, 0).
+struct GridFrame { float lo[3], scale[3]; };
+
+__device__ __forceinline__ uint32_t node_ref(const hcc_node &nd, uint32_t rank) {
+    return nd.count == 0 ? rank + 1u : (HCC_REF_LEAF | ((nd.count - 1u) << 28) | nd.left_or_first);
+}
+
+__global__ void k_build_qrec(const hcc_node *__restrict__ nodes, const uint32_t *__restrict__ internal,
+                             const uint32_t *__restrict__ rank, uint32_t n_internal, GridFrame f,
+                             uint32_t *__restrict__ qrec) {
+    uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_internal) return;
+    const uint32_t left = nodes[internal[k]].left_or_first;
+    uint32_t w[8];
+    for (uint32_t c = 0; c < 2; ++c) {
+        const hcc_node ch = nodes[left + c];
+        for (int a = 0; a < 3; ++a) {
+            const float gl = (ch.lo[a] - f.lo[a]) * f.scale[a] + HCC_GRID_OFFSET;
+            const float gh = (ch.hi[a] - f.lo[a]) * f.scale[a] + HCC_GRID_OFFSET;
+            // NaN or out-of-range boxes fall back to the whole axis (conservative)
+            int ql = gl >= 1.0f ? (gl < 32768.0f ? (int)floorf(gl) - 1 : 32767) : 0;
+            int qh = gh < 32766.0f ? (gh >= 0.0f ? (int)ceilf(gh) + 1 : 0) : 32767;
+            if (!(gl == gl) || !(gh == gh)) { ql = 0; qh = 32767; }
+            w[3 * c + a] = (uint32_t)ql | ((uint32_t)qh << 16);
+        }
+        w[6 + c] = node_ref(ch, rank[left + c]);
+    }
+    uint4 *out = reinterpret_cast<uint4 *>(qrec + 8 * (size_t)k);
+    out[0] = make_uint4(w[0], w[1], w[2], w[3]);
+    out[1] = make_uint4(w[4], w[5], w[6], w[7]);
+}
+
+// Triangle record k (leaf order), 64 bytes so that it is two aligned 256-bit loads:
+// (v0, prim id), (e1 = v1 - v0, 0), (e2 = v2 - v0, 0), padding.
 __global__ void k_convert_tris(const float *__restrict__ tris, const uint32_t *__restrict__ prim_idx,
                                uint32_t n, float4 *__restrict__ out) {
     uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -58,9 +86,10 @@ __global__ void k_convert_tris(const float *__restrict__ tris, const uint32_t *_
     uint32_t id = prim_idx[k];
     const float *v = tris + 9 * (size_t)id;
     float v0x = v[0], v0y = v[1], v0z = v[2];
-    out[3 * (size_t)k + 0] = make_float4(v0x, v0y, v0z, __uint_as_float(id));
-    out[3 * (size_t)k + 1] = make_float4(v[3] - v0x, v[4] - v0y, v[5] - v0z, 0.0f);
-    out[3 * (size_t)k + 2] = make_float4(v[6] - v0x, v[7] - v0y, v[8] - v0z, 0.0f);
+    out[4 * (size_t)k + 0] = make_float4(v0x, v0y, v0z, __uint_as_float(id));
+    out[4 * (size_t)k + 1] = make_float4(v[3] - v0x, v[4] - v0y, v[5] - v0z, 0.0f);
+    out[4 * (size_t)k + 2] = make_float4(v[6] - v0x, v[7] - v0y, v[8] - v0z, 0.0f);
+    out[4 * (size_t)k + 3] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
 }
 
 // Bottom-up pass: one thread per leaf walks to the root; at each parent the second
@@ -125,7 +154,9 @@ extern "C" int32_t hcc_bvh_destroy(hcc_bvh *b) {
     cudaFree(b->d_leaves);
     cudaFree(b->d_flags);
     cudaFree(b->d_internal);
-    cudaFree(b->d_trec);
+    cudaFree(b->d_qrec);
+    cudaFree(b->d_trace_ctl);
+    delete b->trace_calls;
     cudaFree(b->d_ttri);
     delete b;
     return HCC_OK;
@@ -180,8 +211,21 @@ extern "C" int32_t hcc_bvh_create(const hcc_node *nodes, uint32_t n_nodes, const
     b->n_nodes = n_nodes; b->n_tris = n_tris; b->n_leaves = n_leaves; b->max_depth = max_depth;
     for (int a = 0; a < 3; ++a) { b->scene_lo[a] = nodes[0].lo[a]; b->scene_hi[a] = nodes[0].hi[a]; }
 
+    // traversal grid over the root box and the root's traversal reference
+    GridFrame frame;
+    for (int a = 0; a < 3; ++a) {
+        const float ext = b->scene_hi[a] - b->scene_lo[a];
+        b->q_lo[a] = frame.lo[a] = b->scene_lo[a];
+        b->q_scale[a] = frame.scale[a] = ext > 0.0f && HCC_GRID_CELLS / ext < 3.0e38f ? HCC_GRID_CELLS / ext : 0.0f;
+    }
+    b->n_internal = (uint32_t)internal_ids.size();
+    b->trace_calls = new std::atomic<uint32_t>(0u);
+    b->root_ref = nodes[0].count == 0 ? 1u : (HCC_REF_LEAF | ((nodes[0].count - 1u) << 28) | nodes[0].left_or_first);
+    std::vector<uint32_t> rank(n_nodes, 0u);     // rank of an internal node among the internal nodes
+    for (uint32_t k = 0; k < b->n_internal; ++k) rank[internal_ids[k]] = k;
+
     float *d_tris = nullptr;
-    uint32_t *d_prim = nullptr;
+    uint32_t *d_prim = nullptr, *d_rank = nullptr;
     cudaError_t e = cudaSuccess;
     auto alloc = [&](void **p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
     alloc((void **)&b->d_nodes, sizeof(hcc_node) * (size_t)n_nodes);
@@ -189,36 +233,43 @@ extern "C" int32_t hcc_bvh_create(const hcc_node *nodes, uint32_t n_nodes, const
     alloc((void **)&b->d_leaves, sizeof(uint32_t) * (size_t)n_nodes);
     alloc((void **)&b->d_flags, sizeof(uint32_t) * (size_t)n_nodes);
     alloc((void **)&b->d_internal, sizeof(uint32_t) * (internal_ids.size() + 1));
-    alloc((void **)&b->d_trec, sizeof(float4) * 2 * ((size_t)n_nodes + 1));
-    alloc((void **)&b->d_ttri, sizeof(float4) * 3 * (size_t)n_tris);
+    alloc((void **)&b->d_qrec, 32 * (internal_ids.size() + 1));
+    alloc((void **)&b->d_trace_ctl, 2 * 256 * sizeof(uint32_t));
+    alloc((void **)&b->d_ttri, sizeof(float4) * 4 * (size_t)n_tris);
+    alloc((void **)&d_rank, sizeof(uint32_t) * (size_t)n_nodes);
     alloc((void **)&d_tris, sizeof(float) * 9 * (size_t)n_tris);
     alloc((void **)&d_prim, sizeof(uint32_t) * (size_t)n_tris);
     if (e != cudaSuccess) {
         set_error("hcc_bvh_create: cudaMalloc failed: %s", cudaGetErrorString(e));
-        cudaFree(d_tris); cudaFree(d_prim);
+        cudaFree(d_tris); cudaFree(d_prim); cudaFree(d_rank);
         hcc_bvh_destroy(b);
         return e == cudaErrorMemoryAllocation ? HCC_ERR_OUT_OF_MEMORY : HCC_ERR_CUDA;
     }
     auto fail = [&](cudaError_t err, const char *what) {
         set_error("hcc_bvh_create: %s: %s", what, cudaGetErrorString(err));
-        cudaFree(d_tris); cudaFree(d_prim);
+        cudaFree(d_tris); cudaFree(d_prim); cudaFree(d_rank);
         hcc_bvh_destroy(b);
         return (int32_t)HCC_ERR_CUDA;
     };
     if ((e = cudaMemcpyAsync(b->d_nodes, nodes, sizeof(hcc_node) * (size_t)n_nodes, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy nodes");
     if ((e = cudaMemcpyAsync(d_tris, tris, sizeof(float) * 9 * (size_t)n_tris, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy triangles");
     if ((e = cudaMemcpyAsync(d_prim, prim_idx, sizeof(uint32_t) * (size_t)n_tris, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy prim_idx");
+    if ((e = cudaMemcpyAsync(d_rank, rank.data(), sizeof(uint32_t) * (size_t)n_nodes, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy ranks");
     if (!internal_ids.empty() &&
         (e = cudaMemcpyAsync(b->d_internal, internal_ids.data(), sizeof(uint32_t) * internal_ids.size(), cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy internal ids");
     if ((e = cudaMemsetAsync(b->d_flags, 0, sizeof(uint32_t) * (size_t)n_nodes, s)) != cudaSuccess) return fail(e, "memset");
+    if ((e = cudaMemsetAsync(b->d_trace_ctl, 0, 2 * 256 * sizeof(uint32_t), s)) != cudaSuccess) return fail(e, "memset");
     const uint32_t T = 256;
-    k_convert_nodes<<<(n_nodes + T - 1) / T, T, 0, s>>>(b->d_nodes, n_nodes, b->d_trec, b->d_parent);
+    k_parents<<<(n_nodes + T - 1) / T, T, 0, s>>>(b->d_nodes, n_nodes, b->d_parent);
+    if (b->n_internal)
+        k_build_qrec<<<(b->n_internal + T - 1) / T, T, 0, s>>>(b->d_nodes, b->d_internal, d_rank, b->n_internal, frame, b->d_qrec);
     k_convert_tris<<<(n_tris + T - 1) / T, T, 0, s>>>(d_tris, d_prim, n_tris, b->d_ttri);
     k_subtree_leaves<<<(n_nodes + T - 1) / T, T, 0, s>>>(b->d_nodes, b->d_parent, b->d_flags, n_nodes, b->d_leaves);
     if ((e = cudaGetLastError()) != cudaSuccess) return fail(e, "conversion kernels");
     if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return fail(e, "synchronise");
     cudaFree(d_tris);
     cudaFree(d_prim);
+    cudaFree(d_rank);
     *out = b;
     return HCC_OK;
 }

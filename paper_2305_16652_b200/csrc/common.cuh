@@ -5,6 +5,8 @@
 #include <stdint.h>
 #include <stdio.h>
 
+#include <atomic>
+
 #include "../../include/hcc.h"
 
 namespace hcc {
@@ -43,6 +45,12 @@ inline int sm_count() {
 
 inline uint64_t round_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
 
+// Traversal grid (bvh.cu, trace.cu): child boxes are stored as 15-bit cell indices of a
+// uniform grid over the root box, rounded outwards and padded by one cell.
+constexpr float HCC_GRID_CELLS = 32763.0f;
+constexpr float HCC_GRID_OFFSET = 2.0f;
+constexpr uint32_t HCC_REF_LEAF = 0x80000000u;
+
 // Device-side level tables of a cut hierarchy, passed to kernels by value.
 struct CutDev {
     uint32_t m;                        // number of levels
@@ -68,8 +76,13 @@ struct hcc_bvh {
     uint32_t *d_leaves;     // sub-tree leaf counts
     uint32_t *d_flags;      // arrival counters of the bottom-up passes
     uint32_t *d_internal;   // indices of the internal nodes, ascending
-    float4 *d_trec;         // traversal records: 2 float4 per node at index (i+1)
-    float4 *d_ttri;         // 3 float4 per triangle, leaf order
+    uint32_t *d_qrec;       // traversal records: 8 words (32 bytes) per INTERNAL node, in node order
+    float4 *d_ttri;         // 4 float4 (64 bytes) per triangle, leaf order
+    uint32_t n_internal;
+    uint32_t root_ref;      // traversal reference of the root (see bvh.cu)
+    uint32_t *d_trace_ctl;  // 256 x {next rank, CTAs done}: work counters of trace launches in flight
+    std::atomic<uint32_t> *trace_calls;
+    float q_lo[3], q_scale[3];   // traversal grid: g = (x - q_lo) * q_scale + HCC_GRID_OFFSET
     // scratch for hcc_select_cut_flat lives in the caller's workspace
 };
 

@@ -1,14 +1,25 @@
 // (a4) trace: software BVH traversal of the (re)ordered rays — PAPER.md:247 ("the trace
-// kernel fetches the rays based on these sorted indices"), :62-64.  B200 has no RT cores;
-// closest-hit and any-hit are hand-written while-while traversal kernels over 32-byte child
-// records (sibling pair = one aligned 64-byte fetch through the read-only path) with a
-// per-thread stack.  Compiled with -fmad=false; fmaf() appears exactly where hcc.h states it.
+// kernel fetches the rays based on these sorted indices"), :62-64.  B200 has no RT cores.
+//
+// Design: persistent warps pull 32-ray chunks of the (sorted) order from an
+// atomic counter and refill finished lanes from the same chunk, so the rays of a warp stay
+// neighbours in the sorted order; each traversal step fetches ONE 32-byte record holding both
+// quantised child boxes (bvh.cu) with a 256-bit load; the warp alternates between a node phase
+// and a triangle phase, each running while at least half of the live lanes take part (a
+// thresholded while-while loop); the stack lives in shared memory (conflict-free, 16 deep) and
+// spills to local memory below that.  Compiled with -fmad=false; fmaf() appears exactly where
+// hcc.h states it for the triangle predicate, which alone defines the results.
 #include "common.cuh"
 
 namespace hcc {
 
 constexpr int TRACE_THREADS = 128;
-constexpr int STACK_SIZE = 64;
+constexpr int TRACE_BLOCKS_PER_SM = 8;
+constexpr int SMEM_STACK = 16;          // entries per thread in shared memory
+constexpr int STACK_SIZE = 64;          // hcc_bvh_create admits depth <= 63
+constexpr uint32_t CHUNK = 32;          // rays a warp takes from the counter at a time
+constexpr uint32_t REFILL_AT = 8;       // idle lanes that trigger a refill
+constexpr int TRACE_SLOTS = 256;        // counter slots per BVH (traces in flight at once)
 
 __device__ __forceinline__ float max3(float a, float b, float c) {
     float d;
@@ -21,22 +32,27 @@ __device__ __forceinline__ float min3(float a, float b, float c) {
     return d;
 }
 
-struct Ray {
-    float ox, oy, oz, tmin, dx, dy, dz, tmax, ix, iy, iz;
-};
-
-// Conservative culling test on [tmin, limit]: slab distances (lo-o)*inv, (hi-o)*inv, the far
-// end widened by 2 ulp so rounding can never cull a box whose triangle the predicate accepts.
-// A box whose near distance equals `limit` is kept (ties in t go to the lowest prim id).
-__device__ __forceinline__ bool box_hit(const Ray &r, const float4 lo, const float4 hi, float limit, float &tn) {
-    float t1x = (lo.x - r.ox) * r.ix, t2x = (hi.x - r.ox) * r.ix;
-    float t1y = (lo.y - r.oy) * r.iy, t2y = (hi.y - r.oy) * r.iy;
-    float t1z = (lo.z - r.oz) * r.iz, t2z = (hi.z - r.oz) * r.iz;
-    tn = fmaxf(max3(fminf(t1x, t2x), fminf(t1y, t2y), fminf(t1z, t2z)), r.tmin);
-    float tf = min3(fmaxf(t1x, t2x), fmaxf(t1y, t2y), fmaxf(t1z, t2z)) * 1.0000002384185791015625f;
-    tf = fminf(tf, limit);
-    return tn <= tf;
+// One grid cell index (15 bits, low or high half of w, chosen by the byte selector) -> the
+// float 32768 + cell, in one PRMT: bytes {0x00, cell.lo, cell.hi, 0x47}.
+__device__ __forceinline__ float cell_plane(uint32_t w, uint32_t sel) {
+    uint32_t d;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(w), "r"(0x47000000u), "r"(sel));
+    return __uint_as_float(d);
 }
+constexpr uint32_t SEL_LO = 0x7104u, SEL_HI = 0x7324u, SEL_FLIP = 0x0220u;
+
+struct Words8 { uint32_t w[8]; };
+__device__ __forceinline__ Words8 ld256(const uint32_t *p) {   // LDG.E.256 through the read-only path
+    Words8 r;
+    asm volatile("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(r.w[0]), "=r"(r.w[1]), "=r"(r.w[2]), "=r"(r.w[3]), "=r"(r.w[4]), "=r"(r.w[5]), "=r"(r.w[6]), "=r"(r.w[7])
+                 : "l"(p));
+    return r;
+}
+
+struct Ray {
+    float ox, oy, oz, tmin, dx, dy, dz, tmax;
+};
 
 // The triangle predicate of hcc.h, operation by operation.
 __device__ __forceinline__ bool tri_hit(const Ray &r, const float4 v0, const float4 e1, const float4 e2,
@@ -59,90 +75,184 @@ __device__ __forceinline__ bool tri_hit(const Ray &r, const float4 v0, const flo
     return t > r.tmin && t < r.tmax;
 }
 
-// STATS: the same traversal also counts, per ray, the sibling pairs fetched (64 bytes each) and
-// the triangle records fetched (48 bytes each), summed into stats[0], stats[1]; stats[2] = rays,
-// stats[3] = deepest stack seen.  Used for the "node bytes per ray" figure only, never timed.
+struct TraceScene {
+    const uint32_t *qrec;
+    const float4 *ttri;
+    uint32_t root_ref;
+    float q_lo[3], q_scale[3];
+};
+
+// ctl[0] = next ray rank, ctl[1] = CTAs finished (the last one re-arms both for the next launch).
+// STATS: the same traversal also counts the pair records fetched (32 bytes each) and the
+// triangle records fetched (64 bytes each): stats[0], stats[1]; stats[2] = rays, stats[3] =
+// deepest stack seen.  Used for the "bytes per ray" figures only, never timed.
 template <bool ANY, bool STATS>
-__global__ void __launch_bounds__(TRACE_THREADS)
-k_trace(const float4 *__restrict__ trec, const float4 *__restrict__ ttri, const float4 *__restrict__ rays,
-        const uint32_t *__restrict__ perm, uint32_t n, void *__restrict__ hits, unsigned long long *stats) {
-    uint32_t n_pairs = 0, n_tris = 0, max_sp = 0;
-    const uint32_t j = blockIdx.x * TRACE_THREADS + threadIdx.x;
-    if (j >= n) return;
-    const uint32_t rid = perm ? perm[j] : j;
-    const float4 a = __ldg(rays + 2 * (size_t)rid), b = __ldg(rays + 2 * (size_t)rid + 1);
-    Ray r;
-    r.ox = a.x; r.oy = a.y; r.oz = a.z; r.tmin = a.w;
-    r.dx = b.x; r.dy = b.y; r.dz = b.z; r.tmax = b.w;
-    r.ix = 1.0f / b.x; r.iy = 1.0f / b.y; r.iz = 1.0f / b.z;
+__global__ void __launch_bounds__(TRACE_THREADS, TRACE_BLOCKS_PER_SM)
+k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__restrict__ perm, uint32_t n,
+        void *__restrict__ hits, uint32_t *ctl, unsigned long long *stats) {
+    __shared__ uint32_t s_stack[SMEM_STACK][TRACE_THREADS];
+    uint32_t l_stack[STACK_SIZE - SMEM_STACK];
+    const uint32_t tid = threadIdx.x, lane = tid & 31u;
+    const uint32_t lanes_below = (1u << lane) - 1u;
+    unsigned long long n_pairs = 0, n_tris = 0, n_rays = 0;
+    uint32_t max_sp = 0;
 
-    float best_t = r.tmax, best_u = 0.0f, best_v = 0.0f;   // culling limit; the hit's t once one is found
-    uint32_t best_prim = HCC_MISS_PRIM;
-    bool occluded = false;
-
-    uint32_t stack[STACK_SIZE];
+    uint32_t w_next = 0, w_end = 0;      // the warp's current chunk of ranks
+    bool exhausted = false, have = false;
+    uint32_t cur = 0, rid = 0;           // cur: 0 = ray finished, else a record reference
     int sp = 0;
-    uint32_t cur;
-    {   // root = record 1
-        const float4 lo = __ldg(trec + 2), hi = __ldg(trec + 3);
-        float tn;
-        cur = box_hit(r, lo, hi, best_t, tn) ? __float_as_uint(lo.w) : 0u;   // 0 = nothing to do
-    }
-    while (cur != 0u) {
-        // descend through internal nodes: cur = record index of a sibling pair's left child
-        while (!(cur & 0x80000000u)) {
-            const float4 *p = trec + 2 * (size_t)cur;
-            const float4 l_lo = __ldg(p), l_hi = __ldg(p + 1), r_lo = __ldg(p + 2), r_hi = __ldg(p + 3);
-            if (STATS) ++n_pairs;
-            float tn0, tn1;
-            const bool h0 = box_hit(r, l_lo, l_hi, best_t, tn0);
-            const bool h1 = box_hit(r, r_lo, r_hi, best_t, tn1);
-            const uint32_t ref0 = __float_as_uint(l_lo.w), ref1 = __float_as_uint(r_lo.w);
-            if (h0 && h1) {
-                const bool swap = tn1 < tn0;
-                stack[sp++] = swap ? ref0 : ref1;
-                if (STATS) max_sp = max(max_sp, (uint32_t)sp);
-                cur = swap ? ref1 : ref0;
-            } else if (h0) {
-                cur = ref0;
-            } else if (h1) {
-                cur = ref1;
-            } else {
-                cur = sp > 0 ? stack[--sp] : 0u;
-                if (cur == 0u) break;
+    Ray r;
+    float ix = 0.f, iy = 0.f, iz = 0.f, cx = 0.f, cy = 0.f, cz = 0.f;   // slab planes: t = (32768+cell)*i + c
+    uint32_t snx = SEL_LO, sny = SEL_LO, snz = SEL_LO;                  // near-plane selectors
+    float best_t = 0.f, best_u = 0.f, best_v = 0.f;                     // culling limit / the hit
+    uint32_t best_prim = HCC_MISS_PRIM;
+
+    auto push = [&](uint32_t v) {
+        if (sp < SMEM_STACK) s_stack[sp][tid] = v; else l_stack[sp - SMEM_STACK] = v;
+        ++sp;
+        if (STATS) max_sp = max(max_sp, (uint32_t)sp);
+    };
+    auto pop = [&]() -> uint32_t {
+        if (sp == 0) return 0u;
+        --sp;
+        return sp < SMEM_STACK ? s_stack[sp][tid] : l_stack[sp - SMEM_STACK];
+    };
+
+    for (;;) {
+        // ---- refill idle lanes with the next ranks of the warp's chunk
+        uint32_t idle = __ballot_sync(0xFFFFFFFFu, !have);
+        if (!exhausted && (idle == 0xFFFFFFFFu || (uint32_t)__popc(idle) >= REFILL_AT)) {
+            while (idle) {
+                if (w_next == w_end) {
+                    uint32_t base = 0;
+                    if (lane == 0) base = atomicAdd(&ctl[0], CHUNK);
+                    base = __shfl_sync(0xFFFFFFFFu, base, 0);
+                    if (base >= n) { exhausted = true; break; }
+                    w_next = base;
+                    w_end = min(base + CHUNK, n);
+                }
+                const uint32_t avail = w_end - w_next;
+                const uint32_t rank = __popc(idle & lanes_below);
+                if (!have && rank < avail) {
+                    const uint32_t j = w_next + rank;
+                    rid = perm ? perm[j] : j;
+                    const float4 a = __ldg(rays + 2 * (size_t)rid), b = __ldg(rays + 2 * (size_t)rid + 1);
+                    r.ox = a.x; r.oy = a.y; r.oz = a.z; r.tmin = a.w;
+                    r.dx = b.x; r.dy = b.y; r.dz = b.z; r.tmax = b.w;
+                    // the ray in grid units: g(t) = go + t * (d * scale); a zero (or denormal)
+                    // direction component becomes a huge finite reciprocal so that no inf - inf
+                    // arises: the ray then just does not move along that axis
+                    const float BIG = 1.2676506e30f;   // 2^100
+                    const float gx = (a.x - sc.q_lo[0]) * sc.q_scale[0] + HCC_GRID_OFFSET;
+                    const float gy = (a.y - sc.q_lo[1]) * sc.q_scale[1] + HCC_GRID_OFFSET;
+                    const float gz = (a.z - sc.q_lo[2]) * sc.q_scale[2] + HCC_GRID_OFFSET;
+                    ix = 1.0f / (b.x * sc.q_scale[0]); iy = 1.0f / (b.y * sc.q_scale[1]); iz = 1.0f / (b.z * sc.q_scale[2]);
+                    ix = ix == ix ? fminf(fmaxf(ix, -BIG), BIG) : BIG;
+                    iy = iy == iy ? fminf(fmaxf(iy, -BIG), BIG) : BIG;
+                    iz = iz == iz ? fminf(fmaxf(iz, -BIG), BIG) : BIG;
+                    cx = -fmaf(gx, ix, 32768.0f * ix); cy = -fmaf(gy, iy, 32768.0f * iy); cz = -fmaf(gz, iz, 32768.0f * iz);
+                    snx = ix >= 0.0f ? SEL_LO : SEL_HI; sny = iy >= 0.0f ? SEL_LO : SEL_HI; snz = iz >= 0.0f ? SEL_LO : SEL_HI;
+                    best_t = r.tmax; best_u = 0.f; best_v = 0.f; best_prim = HCC_MISS_PRIM;
+                    sp = 0;
+                    cur = sc.root_ref;
+                    have = true;
+                    if (STATS) ++n_rays;
+                }
+                w_next += min((uint32_t)__popc(idle), avail);
+                idle = __ballot_sync(0xFFFFFFFFu, !have);
             }
         }
-        if (cur == 0u) break;
-        // leaf: test its triangles
-        const uint32_t first = cur & 0x0FFFFFFFu, cnt = ((cur >> 28) & 7u) + 1u;
-        for (uint32_t k = 0; k < cnt; ++k) {
-            const float4 *tp = ttri + 3 * (size_t)(first + k);
-            const float4 v0 = __ldg(tp), e1 = __ldg(tp + 1), e2 = __ldg(tp + 2);
-            float t, u, v;
-            if (STATS) ++n_tris;
-            if (tri_hit(r, v0, e1, e2, t, u, v)) {
-                if (ANY) { occluded = true; break; }
-                const uint32_t prim = __float_as_uint(v0.w);
-                if (t < best_t || (t == best_t && prim < best_prim)) {
-                    best_t = t; best_u = u; best_v = v; best_prim = prim;
+        if (__ballot_sync(0xFFFFFFFFu, have) == 0u) break;
+
+        // ---- node phase: while at least half of the live lanes want a node step
+        {
+            uint32_t m = __ballot_sync(0xFFFFFFFFu, cur != 0u && !(cur & HCC_REF_LEAF));
+            const uint32_t live = __popc(__ballot_sync(0xFFFFFFFFu, cur != 0u));
+            const uint32_t need = (live + 1u) / 2u;
+            while (m != 0u && (uint32_t)__popc(m) >= need) {
+                if (cur != 0u && !(cur & HCC_REF_LEAF)) {
+                    const Words8 q = ld256(sc.qrec + 8 * (size_t)(cur - 1u));
+                    if (STATS) ++n_pairs;
+                    const uint32_t sfx = snx ^ SEL_FLIP, sfy = sny ^ SEL_FLIP, sfz = snz ^ SEL_FLIP;
+                    float tn0 = max3(fmaf(cell_plane(q.w[0], snx), ix, cx), fmaf(cell_plane(q.w[1], sny), iy, cy), fmaf(cell_plane(q.w[2], snz), iz, cz));
+                    float tf0 = min3(fmaf(cell_plane(q.w[0], sfx), ix, cx), fmaf(cell_plane(q.w[1], sfy), iy, cy), fmaf(cell_plane(q.w[2], sfz), iz, cz));
+                    float tn1 = max3(fmaf(cell_plane(q.w[3], snx), ix, cx), fmaf(cell_plane(q.w[4], sny), iy, cy), fmaf(cell_plane(q.w[5], snz), iz, cz));
+                    float tf1 = min3(fmaf(cell_plane(q.w[3], sfx), ix, cx), fmaf(cell_plane(q.w[4], sfy), iy, cy), fmaf(cell_plane(q.w[5], sfz), iz, cz));
+                    tn0 = fmaxf(tn0, r.tmin); tn1 = fmaxf(tn1, r.tmin);
+                    tf0 = fminf(tf0, best_t); tf1 = fminf(tf1, best_t);     // a box starting AT best_t is kept
+                    const bool h0 = tn0 <= tf0, h1 = tn1 <= tf1;
+                    const uint32_t ref0 = q.w[6], ref1 = q.w[7];
+                    if (h0 && h1) {
+                        const bool swap = tn1 < tn0;
+                        push(swap ? ref0 : ref1);
+                        cur = swap ? ref1 : ref0;
+                    } else if (h0) cur = ref0;
+                    else if (h1) cur = ref1;
+                    else cur = pop();
+                }
+                m = __ballot_sync(0xFFFFFFFFu, cur != 0u && !(cur & HCC_REF_LEAF));
+            }
+        }
+        // ---- triangle phase
+        if (ANY) {
+            // one triangle per lane per iteration, while a quarter of the live lanes hold a leaf
+            uint32_t m = __ballot_sync(0xFFFFFFFFu, (cur & HCC_REF_LEAF) != 0u);
+            const uint32_t live = __popc(__ballot_sync(0xFFFFFFFFu, cur != 0u));
+            const uint32_t need = (live + 3u) / 4u;
+            while (m != 0u && (uint32_t)__popc(m) >= need) {
+                if (cur & HCC_REF_LEAF) {
+                    const uint32_t first = cur & 0x0FFFFFFFu, rem = (cur >> 28) & 7u;
+                    const Words8 A = ld256(reinterpret_cast<const uint32_t *>(sc.ttri + 4 * (size_t)first));
+                    const float4 e2 = __ldg(sc.ttri + 4 * (size_t)first + 2);
+                    if (STATS) ++n_tris;
+                    const float4 v0 = make_float4(__uint_as_float(A.w[0]), __uint_as_float(A.w[1]), __uint_as_float(A.w[2]), 0.f);
+                    const float4 e1 = make_float4(__uint_as_float(A.w[4]), __uint_as_float(A.w[5]), __uint_as_float(A.w[6]), 0.f);
+                    float t, u, v;
+                    if (tri_hit(r, v0, e1, e2, t, u, v)) { best_prim = 0u; sp = 0; cur = 0u; }
+                    else cur = rem == 0u ? pop() : (HCC_REF_LEAF | ((rem - 1u) << 28) | (first + 1u));
+                }
+                m = __ballot_sync(0xFFFFFFFFu, (cur & HCC_REF_LEAF) != 0u);
+            }
+        } else if (cur & HCC_REF_LEAF) {
+            const uint32_t first = cur & 0x0FFFFFFFu, cnt = ((cur >> 28) & 7u) + 1u;
+            for (uint32_t k = 0; k < cnt; ++k) {
+                const float4 *tp = sc.ttri + 4 * (size_t)(first + k);
+                const Words8 A = ld256(reinterpret_cast<const uint32_t *>(tp));
+                const float4 e2 = __ldg(tp + 2);
+                if (STATS) ++n_tris;
+                const float4 v0 = make_float4(__uint_as_float(A.w[0]), __uint_as_float(A.w[1]), __uint_as_float(A.w[2]), 0.f);
+                const float4 e1 = make_float4(__uint_as_float(A.w[4]), __uint_as_float(A.w[5]), __uint_as_float(A.w[6]), 0.f);
+                float t, u, v;
+                if (tri_hit(r, v0, e1, e2, t, u, v)) {
+                    const uint32_t prim = A.w[3];
+                    if (t < best_t || (t == best_t && prim < best_prim)) { best_t = t; best_u = u; best_v = v; best_prim = prim; }
                 }
             }
+            cur = pop();
         }
-        if (ANY && occluded) break;
-        cur = sp > 0 ? stack[--sp] : 0u;
+        __syncwarp();
+        // ---- retire finished rays
+        if (have && cur == 0u) {
+            if (ANY) reinterpret_cast<uint8_t *>(hits)[rid] = best_prim != HCC_MISS_PRIM ? 1 : 0;
+            else {
+                const bool hit = best_prim != HCC_MISS_PRIM;
+                reinterpret_cast<float4 *>(hits)[rid] =
+                    make_float4(hit ? best_t : __int_as_float(0x7f800000), __uint_as_float(best_prim), best_u, best_v);
+            }
+            have = false;
+        }
     }
     if (STATS) {
-        atomicAdd(&stats[0], (unsigned long long)n_pairs);
-        atomicAdd(&stats[1], (unsigned long long)n_tris);
-        atomicAdd(&stats[2], 1ull);
+        atomicAdd(&stats[0], n_pairs);
+        atomicAdd(&stats[1], n_tris);
+        atomicAdd(&stats[2], n_rays);
         atomicMax(&stats[3], (unsigned long long)max_sp);
     }
-    if (ANY) {
-        reinterpret_cast<uint8_t *>(hits)[rid] = occluded ? 1 : 0;
-    } else {
-        const bool hit = best_prim != HCC_MISS_PRIM;
-        reinterpret_cast<float4 *>(hits)[rid] =
-            make_float4(hit ? best_t : __int_as_float(0x7f800000), __uint_as_float(best_prim), best_u, best_v);
+    // the last CTA to finish re-arms the counters for the next launch on this slot
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        if (atomicAdd(&ctl[1], 1u) == gridDim.x - 1u) { ctl[0] = 0u; ctl[1] = 0u; __threadfence(); }
     }
 }
 
@@ -160,18 +270,21 @@ static int32_t trace_impl(const char *who, const hcc_bvh *bvh, const float *rays
                 "%s: rays need 32-byte, hits and perm 16-byte alignment", who);
     HCC_REQUIRE(n < (1ull << 32), HCC_ERR_UNSUPPORTED, "%s: n >= 2^32", who);
     cudaStream_t s = (cudaStream_t)stream;
-    const uint32_t blocks = (uint32_t)((n + TRACE_THREADS - 1) / TRACE_THREADS);
+    const uint32_t cap = (uint32_t)sm_count() * TRACE_BLOCKS_PER_SM;
+    const uint32_t want = (uint32_t)((n + TRACE_THREADS - 1) / TRACE_THREADS);
+    const uint32_t blocks = want < cap ? want : cap;
+    TraceScene sc;
+    sc.qrec = bvh->d_qrec; sc.ttri = bvh->d_ttri; sc.root_ref = bvh->root_ref;
+    for (int a = 0; a < 3; ++a) { sc.q_lo[a] = bvh->q_lo[a]; sc.q_scale[a] = bvh->q_scale[a]; }
+    // every launch takes the next counter slot; slots re-arm themselves (see the kernel's end)
+    uint32_t *ctl = bvh->d_trace_ctl + 2u * (bvh->trace_calls->fetch_add(1u) % (uint32_t)TRACE_SLOTS);
     const float4 *rays = (const float4 *)rays_dev;
     if (stats_dev) {
-        if (mode == HCC_TRACE_CLOSEST)
-            k_trace<false, true><<<blocks, TRACE_THREADS, 0, s>>>(bvh->d_trec, bvh->d_ttri, rays, perm_dev, (uint32_t)n, hits_dev, stats_dev);
-        else
-            k_trace<true, true><<<blocks, TRACE_THREADS, 0, s>>>(bvh->d_trec, bvh->d_ttri, rays, perm_dev, (uint32_t)n, hits_dev, stats_dev);
+        if (mode == HCC_TRACE_CLOSEST) k_trace<false, true><<<blocks, TRACE_THREADS, 0, s>>>(sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, stats_dev);
+        else                           k_trace<true, true><<<blocks, TRACE_THREADS, 0, s>>>(sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, stats_dev);
     } else {
-        if (mode == HCC_TRACE_CLOSEST)
-            k_trace<false, false><<<blocks, TRACE_THREADS, 0, s>>>(bvh->d_trec, bvh->d_ttri, rays, perm_dev, (uint32_t)n, hits_dev, nullptr);
-        else
-            k_trace<true, false><<<blocks, TRACE_THREADS, 0, s>>>(bvh->d_trec, bvh->d_ttri, rays, perm_dev, (uint32_t)n, hits_dev, nullptr);
+        if (mode == HCC_TRACE_CLOSEST) k_trace<false, false><<<blocks, TRACE_THREADS, 0, s>>>(sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, nullptr);
+        else                           k_trace<true, false><<<blocks, TRACE_THREADS, 0, s>>>(sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, nullptr);
     }
     HCC_CUDA_TRY(cudaGetLastError());
     return HCC_OK;
