@@ -8,13 +8,24 @@ namespace hcc {
 
 constexpr int RADIX_BITS = 8;
 constexpr int RADIX = 1 << RADIX_BITS;
-constexpr int SORT_THREADS = 256;            // == RADIX: thread d owns digit d in the scan phases
+#ifndef HCC_SORT_THREADS
+#define HCC_SORT_THREADS 512
+#endif
+#ifndef HCC_SORT_ITEMS
+#define HCC_SORT_ITEMS 8
+#endif
+#ifndef HCC_SORT_MIN_CTAS
+#define HCC_SORT_MIN_CTAS 3
+#endif
+constexpr int SORT_THREADS = HCC_SORT_THREADS;   // >= RADIX: thread d < RADIX owns digit d in the scan phases
 constexpr int SORT_WARPS = SORT_THREADS / 32;
-constexpr int SORT_ITEMS = 16;
+constexpr int SORT_ITEMS = HCC_SORT_ITEMS;
 constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;   // 4096 pairs per CTA
 constexpr int MAX_PASSES = 8;
 constexpr uint32_t FLAG_AGG = 1u << 30, FLAG_PREFIX = 2u << 30, VAL_MASK = (1u << 30) - 1u;
 constexpr int HIST_THREADS = 256;
+constexpr int SORT_MIN_CTAS = HCC_SORT_MIN_CTAS;  // caps the registers: occupancy decides this kernel's speed
+constexpr int LOOK = 4;                      // look-back rows fetched per round trip
 
 // control region of the workspace (zeroed once per sort by one memset)
 struct SortCtl {
@@ -80,13 +91,13 @@ __global__ void k_iota(uint32_t *perm, uint32_t n) {
 // global base.  Tiles are handed out by an atomic ticket so that every predecessor of a
 // running tile is itself running or done (forward progress of the look-back spin).
 template <typename KeyT, bool FIRST, bool WRITE_KEYS>
-__global__ void __launch_bounds__(SORT_THREADS)
+__global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_CTAS)
 k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const uint32_t *__restrict__ vals_in,
            uint32_t *__restrict__ vals_out, uint32_t n, uint32_t shift, uint32_t *status, uint32_t *ticket) {
     __shared__ uint32_t s_warp_hist[SORT_WARPS][RADIX];
     __shared__ uint32_t s_tile_off[RADIX];
     __shared__ uint32_t s_gbase[RADIX];
-    __shared__ uint32_t s_warp_tot[SORT_WARPS];
+    __shared__ uint32_t s_warp_tot[RADIX / 32];
     __shared__ uint32_t s_tile;
     extern __shared__ __align__(16) unsigned char s_dyn[];
     KeyT *s_keys = reinterpret_cast<KeyT *>(s_dyn);
@@ -114,7 +125,15 @@ k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const 
     for (int i = 0; i < SORT_ITEMS; ++i) {
         const bool valid = my_base + 32 * i < count;
         const uint32_t digit = valid ? ((uint32_t)(key[i] >> shift) & (RADIX - 1)) : (uint32_t)RADIX;
-        const uint32_t peers = __match_any_sync(0xFFFFFFFFu, digit);
+        // lanes holding the same digit: one ballot per digit bit (MATCH.ANY costs a round per
+        // distinct value in the warp, far more on well-spread digits)
+        uint32_t peers = 0xFFFFFFFFu;
+#pragma unroll
+        for (int b = 0; b <= RADIX_BITS; ++b) {
+            const bool bit = (digit >> b) & 1u;
+            const uint32_t m = __ballot_sync(0xFFFFFFFFu, bit);
+            peers &= bit ? m : ~m;
+        }
         const uint32_t below = __popc(peers & lt);
         const uint32_t old = s_warp_hist[warp][digit & (RADIX - 1)];
         __syncwarp();
@@ -124,9 +143,11 @@ k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const 
     }
     __syncthreads();
 
-    // thread d: digit d.  Warp-exclusive offsets, tile total, publish, scan over digits, look back.
-    {
-        const uint32_t d = tid;
+    // thread d: digit d.  Warp-exclusive offsets, tile total, publish the aggregate, scan over digits.
+    const uint32_t d = tid;
+    uint32_t total = 0, excl_local = 0, incl = 0;
+    uint32_t *row = status + (size_t)(tile + 1) * RADIX;
+    if (d < RADIX) {
         uint32_t run = 0;
 #pragma unroll
         for (int w = 0; w < SORT_WARPS; ++w) {
@@ -134,37 +155,27 @@ k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const 
             s_warp_hist[w][d] = run;
             run += t;
         }
-        const uint32_t total = run;
-        uint32_t *row = status + (size_t)(tile + 1) * RADIX;
+        total = run;
         st_volatile_u32(row + d, FLAG_AGG | total);
-        uint32_t incl = total;
+        incl = total;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, o);
             if (lane >= (uint32_t)o) incl += x;
         }
         if (lane == 31) s_warp_tot[warp] = incl;
-        __syncthreads();
+    }
+    __syncthreads();
+    if (d < RADIX) {
         uint32_t add = 0;
         for (uint32_t w = 0; w < warp; ++w) add += s_warp_tot[w];
-        const uint32_t excl_local = add + incl - total;
+        excl_local = add + incl - total;
         s_tile_off[d] = excl_local;
-        // decoupled look-back over rows tile, tile-1, ..., 0 (row 0 = seeded global digit base)
-        uint32_t excl = 0;
-        const uint32_t *prow = status + (size_t)tile * RADIX + d;
-        for (;;) {
-            uint32_t v = ld_volatile_u32(prow);
-            if ((v >> 30) == 0u) continue;
-            excl += v & VAL_MASK;
-            if (v & FLAG_PREFIX) break;
-            prow -= RADIX;
-        }
-        st_volatile_u32(row + d, FLAG_PREFIX | ((excl + total) & VAL_MASK));
-        s_gbase[d] = excl - excl_local;
     }
     __syncthreads();
 
-    // scatter into tile order in shared memory
+    // scatter into tile order in shared memory: needs the tile-local offsets only, so it runs
+    // BEFORE the look-back and gives the predecessors time to publish
 #pragma unroll
     for (int i = 0; i < SORT_ITEMS; ++i) {
         const uint32_t idx = my_base + 32 * i;
@@ -174,6 +185,30 @@ k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const 
             s_keys[p] = key[i];
             s_vals[p] = FIRST ? tile_base + idx : vals_in[tile_base + idx];
         }
+    }
+
+    // decoupled look-back over rows tile, tile-1, ..., 0 (row 0 = seeded global digit base).
+    // LOOK rows are read at once: a walk over aggregates costs one L2 round trip per LOOK rows
+    // instead of one per row.  Rows before row 0 are never reached logically (row 0 is a
+    // PREFIX); the speculative reads of them stay inside the workspace.
+    if (d < RADIX) {
+        uint32_t excl = 0;
+        const uint32_t *prow = status + (size_t)tile * RADIX + d;
+        for (bool done = false; !done;) {
+            uint32_t v[LOOK];
+#pragma unroll
+            for (int k = 0; k < LOOK; ++k) v[k] = ld_volatile_u32(prow - (ptrdiff_t)k * RADIX);
+            int k = 0;
+#pragma unroll
+            for (; k < LOOK; ++k) {
+                if ((v[k] >> 30) == 0u) break;
+                excl += v[k] & VAL_MASK;
+                if (v[k] & FLAG_PREFIX) { done = true; break; }
+            }
+            prow -= (ptrdiff_t)k * RADIX;
+        }
+        st_volatile_u32(row + d, FLAG_PREFIX | ((excl + total) & VAL_MASK));
+        s_gbase[d] = excl - excl_local;
     }
     __syncthreads();
     // write out: consecutive threads -> consecutive addresses inside each digit run

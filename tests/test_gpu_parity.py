@@ -372,3 +372,122 @@ def test_error_reporting(hcc, dev_cases):
     cut = hcc.select_cut(d["bvh"], had, 64, 32)
     assert hcc.encode(empty, cut).shape[0] == 0
     assert hcc.trace(d["bvh"], empty, None, hcc.TRACE_ANY).shape[0] == 0
+
+
+# ----------------------------------------------------------------- (a4) edge cases of the traversal
+def _rand_rays(n, seed, lo=-0.2, hi=1.2, axis_parallel=False):
+    """Seeded rays with origins in [lo, hi]^3; with axis_parallel, directions have one or two
+    exactly-zero components (the slab arithmetic's degenerate case)."""
+    from hcc_inputs import rng as hrng
+    u = hrng.u01(seed, 0, np.arange(n, dtype=np.uint64), np.arange(7, dtype=np.uint64)[:, None]).T
+    rays = np.zeros((n, 8), dtype=np.float32)
+    rays[:, 0:3] = lo + (hi - lo) * u[:, 0:3]
+    d = 2.0 * u[:, 3:6] - 1.0
+    if axis_parallel:
+        kill = (u[:, 6] * 6).astype(np.int64)          # 0..5: which components to zero
+        d[kill % 3 == 0, 0] = 0.0
+        d[kill % 3 == 1, 1] = 0.0
+        d[kill >= 3, 2] = 0.0
+        d[np.abs(d).sum(axis=1) == 0, 0] = 1.0
+        d[::7] = np.sign(d[::7]) * (d[::7] != 0)       # exact +-1 axis directions
+        d[(np.abs(d).sum(axis=1) == 0)] = (0.0, -1.0, 0.0)
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    rays[:, 4:7] = d
+    rays[:, 3] = 0.0
+    rays[:, 7] = np.inf
+    return rays
+
+
+def _check_trace_both_modes(hcc, b, rays):
+    import oracle
+    bvh = hcc.Bvh(b.nodes, b.tris, b.prim_idx)
+    rd = torch.from_numpy(rays).cuda()
+    want = oracle.closest_brute(rays, b.tris)
+    got = hcc.hits_to_numpy(hcc.trace(bvh, rd, None, hcc.TRACE_CLOSEST))
+
+    class _C:
+        bvh = b
+    check_closest(_C, rays, got, want)
+    occ = hcc.trace(bvh, rd, None, hcc.TRACE_ANY).cpu().numpy()
+    assert np.array_equal(occ, oracle.any_brute(rays, b.tris))
+    return want
+
+
+def test_trace_axis_parallel_rays_vs_brute_force(hcc, tiny):
+    """Zero direction components: the quantised slab test must neither produce NaN culls nor
+    miss a triangle (hits are defined by the triangle predicate alone)."""
+    rays = _rand_rays(6000 + 13, 0xA11CE, axis_parallel=True)
+    want = _check_trace_both_modes(hcc, tiny.bvh, rays)
+    assert (~np.isinf(want[0])).sum() > 50
+
+
+def test_trace_flat_scene_vs_brute_force(hcc):
+    """All triangles in the plane z = 0.25 (zero scene extent along z): the traversal grid is
+    degenerate on that axis."""
+    import hcc_inputs
+    from hcc_inputs import rng as hrng
+    n = 300
+    u = hrng.u01(0xF1A7, 0, np.arange(n, dtype=np.uint64), np.arange(6, dtype=np.uint64)[:, None]).T
+    tris = np.zeros((n, 3, 3), dtype=np.float32)
+    c = u[:, 0:2]
+    for k in range(3):
+        tris[:, k, 0:2] = c + 0.05 * (u[:, 2 * k % 6:2 * k % 6 + 2] - 0.5)
+    tris[:, :, 2] = 0.25
+    b = hcc_inputs.build_bvh(tris)
+    rays = np.concatenate([_rand_rays(3000, 0xF1A8, lo=0.0, hi=1.0), _rand_rays(1000, 0xF1A9, lo=0.0, hi=1.0, axis_parallel=True)])
+    rays[:, 2] = np.where(np.arange(rays.shape[0]) % 2 == 0, 0.9, -0.4)      # above and below the plane
+    want = _check_trace_both_modes(hcc, b, rays)
+    assert (~np.isinf(want[0])).sum() > 20
+
+
+def test_trace_root_leaf_bvh(hcc):
+    """A BVH that is one leaf (<= 4 triangles): the traversal starts on a leaf reference."""
+    import hcc_inputs
+    tris = np.array([[[0, 0, 0], [1, 0, 0], [0, 1, 0]], [[0, 0, 0.5], [1, 0, 0.5], [0, 1, 0.5]]], dtype=np.float32)
+    b = hcc_inputs.build_bvh(tris)
+    assert b.n_nodes == 1
+    rays = _rand_rays(257, 0x1EAF)
+    rays[:, 0:3] = (0.2, 0.2, 1.0)
+    _check_trace_both_modes(hcc, b, rays)
+
+
+def test_trace_deep_chain_bvh_spills_the_stack(hcc):
+    """A degenerate chain (depth 40 > the 16 shared-memory stack entries) of nested boxes whose
+    far child is always hit too: the per-thread stack spills to local memory and comes back."""
+    import hcc_inputs
+    depth = 40
+    tris, nodes = [], []
+    # node 2k = internal, children (2k+1 = leaf with one triangle, 2k+2 = next internal / last leaf)
+    for k in range(depth + 1):
+        z = 0.02 * (k + 1)
+        tris.append([[0.1, 0.1, z], [0.9, 0.1, z], [0.1, 0.9, z]])
+    for k in range(depth):
+        nodes.append(((0.1, 0.1, 0.02 * (k + 1)), (0.9, 0.9, 0.02 * (depth + 1)), 2 * k + 1, 0))
+        nodes.append(((0.1, 0.1, 0.02 * (k + 1)), (0.9, 0.9, 0.02 * (k + 1)), k, 1))
+    nodes.append(((0.1, 0.1, 0.02 * (depth + 1)), (0.9, 0.9, 0.02 * (depth + 1)), depth, 1))
+    b = hcc_inputs.make_bvh(nodes, np.array(tris, dtype=np.float32))
+    assert b.max_depth == depth
+    # rays travelling in -z from above meet the LAST triangle first: the near child is always the
+    # deeper internal node, so every leaf on the way down is pushed
+    rays = _rand_rays(2000 + 5, 0xDEE9, lo=0.0, hi=1.0)
+    rays[:, 2] = 2.0
+    rays[:, 4:7] = (0.0, 0.0, -1.0)
+    rays[1::2, 4:7] = (0.05, -0.03, -1.0)
+    rays[1::2, 4:7] /= np.linalg.norm(rays[1::2, 4:7], axis=1, keepdims=True)
+    bvh = hcc.Bvh(b.nodes, b.tris, b.prim_idx)
+    st = hcc.trace_stats(bvh, torch.from_numpy(rays).cuda(), None, hcc.TRACE_CLOSEST)
+    assert st["max_stack"] > 16, st
+    _check_trace_both_modes(hcc, b, rays)
+
+
+@pytest.mark.parametrize("n", [1, 31, 32, 33, 127, 129, 4097])
+def test_trace_ragged_sizes_and_counter_rearm(hcc, dev_cases, n):
+    """Ragged batch sizes, and > 256 launches on one BVH (the work-counter slots are reused and
+    must have re-armed themselves)."""
+    d = dev_cases["room_small"]
+    ref = hcc.trace(d["bvh"], d["diffuse"], None, hcc.TRACE_CLOSEST)
+    sub = d["diffuse"][:n].contiguous()
+    reps = 300 if n == 33 else 3
+    for _ in range(reps):
+        got = hcc.trace(d["bvh"], sub, None, hcc.TRACE_CLOSEST)
+    assert torch.equal(got.view(torch.int32), ref[:n].view(torch.int32))
