@@ -38,9 +38,10 @@ UNIT = "Mrays/s"
 
 # Algorithmic work per ray, stated in DESIGN.md "Rooflines":
 #  encode: 32 B ray read + key write;  sort: one histogram read + per pass read+write of (key, id)
-#  trace : fp32 lane-operations = 26 per box test + 36 per triangle test (operation counts of the
-#          formulas in include/hcc.h), box tests = 2 per sibling pair fetched.
-OPS_BOX, OPS_TRI = 26, 36
+#  trace : lane-operations = 34 per sibling-pair record (12 cell->float conversions, 12 fma, 8 min/max,
+#          2 compares: both quantised child boxes, trace.cu) + 36 per triangle test (the formula in
+#          include/hcc.h); encode: 26 per exact fp32 slab test (6 sub, 6 mul, 12 min/max, compare, bit).
+OPS_BOX, OPS_PAIR, OPS_TRI = 26, 34, 36
 SM_COUNT, LANES_PER_SM = 148, 128
 
 
@@ -180,10 +181,12 @@ def run_reference(args):
 
 
 def _config(args, w, n_d, n_s, l2):
-    return {"workload": f"config 2 'room' of BASELINE.json" if args.workload == "room" else args.workload,
+    names = {"room": "config 2 'room' of BASELINE.json", "fig1": "config 3 'Figure-1-like' of BASELINE.json",
+             "large": "config 5 'large' of BASELINE.json", "tiny": "config 1 'tiny' of BASELINE.json"}
+    return {"workload": names[args.workload],
             "triangles": int(w.bvh.n_tris), "bvh_nodes": int(w.bvh.n_nodes), "K": int(w.K),
             "key_bits": int(w.key_bits), "diffuse_rays": int(n_d), "shadow_rays": int(n_s),
-            "resolution": f"{w.width}x{w.height}x{w.spp}spp", "bounce": 1, "l2": l2,
+            "resolution": f"{w.width}x{w.height}x{w.spp}spp", "bounce": int(getattr(args, "bounce", 1)), "l2": l2,
             "parallelism": f"rays sharded over {args.gpus} GPU(s), BVH and cut replicated, no collective"}
 
 
@@ -207,7 +210,7 @@ def run_ours(args):
     hbm_gbs, sm_max_mhz, peak_kind = _peaks()
 
     # ---- inputs (seeded; rank r draws its own sub-pixel samples of the same scene)
-    w = hcc_inputs.Workload(args.workload, rank=rank)
+    w = hcc_inputs.Workload(args.workload, rank=rank, res_scale=args.res_scale)
     b = w.bvh
     bvh = hcc.Bvh(b.nodes, b.tris, b.prim_idx)
 
@@ -216,6 +219,9 @@ def run_ours(args):
         t, p, _, _ = hcc.hits_to_numpy(h)
         return t, p
     diffuse_h, shadow_h = w.first_bounce(gpu_trace_closest)
+    for b_i in range(2, args.bounce + 1):      # later bounces: trace the previous diffuse batch, spawn the next
+        t_prev, p_prev = gpu_trace_closest(None, diffuse_h)
+        diffuse_h, shadow_h, _ = w.bounce(b_i, diffuse_h, t_prev, p_prev)
     n_d, n_s = diffuse_h.shape[0], shadow_h.shape[0]
     n = n_d + n_s
     diffuse = torch.from_numpy(diffuse_h).cuda()
@@ -321,7 +327,7 @@ def run_ours(args):
         perm = hcc.sort(keys, info["bits_used"])
         st = hcc.trace_stats(bvh, rays, perm, mode)
         st0 = hcc.trace_stats(bvh, rays, None, mode)
-        ops = (2 * st["pairs"] * OPS_BOX + st["tris"] * OPS_TRI)
+        ops = (st["pairs"] * OPS_PAIR + st["tris"] * OPS_TRI)
         diag[name] = {"anc_hcc": hcc.anc(keys0, perm), "anc_nosort": hcc.anc(keys0, None),
                       "node_bytes_per_ray": st["node_bytes_per_ray"], "tri_bytes_per_ray": st["tri_bytes_per_ray"],
                       "node_bytes_per_ray_nosort": st0["node_bytes_per_ray"], "max_stack": st["max_stack"],
@@ -351,6 +357,49 @@ def run_ours(args):
             "frac": roof["frac"], "traffic": None, "kernel": f"{dom[1]} ({dom[0]} batch)",
             "peak_source": (f"{peak_kind} HBM copy" if roof["bound"] == "hbm" else
                             f"148 SMs x 128 fp32 lanes x {sm_max_mhz:.0f} MHz (DESIGN.md)")}
+
+    # ---- encode and sort at the batch size of configs 3/5 (the shadow batch tiled to ~33.5 M rays): the
+    #      config-2 batches (1-2 M pairs) are launch- and latency-bound, so the HBM fractions that the
+    #      north_star's 60 % bar is about are measured here (SURVEY.md §7 "hard parts", §8(d))
+    large = None
+    if world == 1 and not args.no_large_n:
+        reps = max(1, (1 << 25) // n_s)
+        big = shadow.repeat(reps, 1) if reps > 1 else shadow
+        nb = big.shape[0]
+        keys_b = hcc.encode(big, cut)
+        keys_b0 = keys_b.clone()
+        ws_b = torch.empty(hcc.sort_workspace_bytes(nb, container), dtype=torch.uint8, device="cuda")
+        perm_b = torch.empty(nb, dtype=torch.int32, device="cuda")
+
+        def med(fn, setup=None, k=7):
+            out = []
+            for i in range(k + 2):
+                if setup:
+                    setup()
+                flush.zero_()
+                s0, e0 = ev(), ev()
+                s0.record(); fn(); e0.record()
+                torch.cuda.synchronize()
+                if i >= 2:
+                    out.append(s0.elapsed_time(e0))
+            return float(np.median(out))
+        enc_ms = med(lambda: hcc.encode(big, cut, keys=keys_b))
+        sort_ms = med(lambda: hcc.sort(keys_b, info["bits_used"], perm=perm_b, workspace=ws_b), setup=lambda: keys_b.copy_(keys_b0))
+        tp_keys = hcc.encode_twopoint(big, bvh.scene_lo, bvh.scene_hi, w.key_bits)
+        tp_ms = med(lambda: hcc.encode_twopoint(big, bvh.scene_lo, bvh.scene_hi, w.key_bits, keys=tp_keys))
+        kb = container // 8
+        eb, sb_ = nb * (32 + kb), nb * (kb + passes * 2 * (kb + 4))
+        tkb = 4 if w.key_bits <= 32 else 8
+        large = {"rays": int(nb), "how": f"shadow batch tiled x{reps}",
+                 "encode": {"ms": enc_ms, "bound": "hbm", "achieved": eb / enc_ms / 1e6, "peak": hbm_gbs, "unit": "GB/s",
+                            "frac": eb / enc_ms / 1e6 / hbm_gbs,
+                            "alu_frac": nb * info["bits_used"] * OPS_BOX / (enc_ms * 1e-3) / 1e12 / (SM_COUNT * LANES_PER_SM * sm_max_mhz * 1e6 / 1e12)},
+                 "sort": {"ms": sort_ms, "bound": "hbm", "achieved": sb_ / sort_ms / 1e6, "peak": hbm_gbs, "unit": "GB/s",
+                          "frac": sb_ / sort_ms / 1e6 / hbm_gbs, "passes": passes},
+                 "encode_twopoint": {"ms": tp_ms, "bound": "hbm", "achieved": nb * (32 + tkb) / tp_ms / 1e6, "peak": hbm_gbs,
+                                     "unit": "GB/s", "frac": nb * (32 + tkb) / tp_ms / 1e6 / hbm_gbs}}
+        del big, keys_b, keys_b0, ws_b, perm_b, tp_keys
+        torch.cuda.empty_cache()
 
     # ---- e2e: the same step through the C ABI with HOST buffers (pinned), copies inside the timing
     rays_pin = {"diffuse": torch.from_numpy(diffuse_h).pin_memory(), "shadow": torch.from_numpy(shadow_h).pin_memory()}
@@ -412,7 +461,8 @@ def run_ours(args):
             "roofline": roof, "cpu_baseline": cpu,
             "cut": {"widths": info["widths"], "K_eff": info["K_eff"], "bits_used": info["bits_used"],
                     "container_bits": container, "cut_ms": cut_ms},
-            "orders": orders, "speedup_hcc": speed, "stages_roofline_hcc": stages, "diagnostics": diag,
+            "orders": orders, "speedup_hcc": speed, "stages_roofline_hcc": stages, "stages_roofline_large_batch": large,
+            "diagnostics": diag,
             "paper_context": "RTX 3060, Breakfast: HCC 67.6 vs NoSort 37.4 vs TwoPoint 56.8 Mrays/s trace-only (PAPER.md:294-299); not comparable"}
     print(json.dumps(line))
     if world > 1:
@@ -430,6 +480,9 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=1 << 20, help="diffuse rays in the cpu_baseline sample")
     ap.add_argument("--ref-sample", type=int, default=1 << 15, help="diffuse rays per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--bounce", type=int, default=1, help="which bounce's ray batches to run (1 = rays off the primary hits)")
+    ap.add_argument("--res-scale", type=float, default=1.0, help="image scale of the workload (1.0 = the config's resolution)")
+    ap.add_argument("--no-large-n", action="store_true", help="skip the large-batch encode/sort roofline leg")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

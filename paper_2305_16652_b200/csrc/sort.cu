@@ -8,30 +8,24 @@ namespace hcc {
 
 constexpr int RADIX_BITS = 8;
 constexpr int RADIX = 1 << RADIX_BITS;
-#ifndef HCC_SORT_THREADS
-#define HCC_SORT_THREADS 512
-#endif
-#ifndef HCC_SORT_ITEMS
-#define HCC_SORT_ITEMS 8
-#endif
-#ifndef HCC_SORT_MIN_CTAS
-#define HCC_SORT_MIN_CTAS 3
-#endif
-constexpr int SORT_THREADS = HCC_SORT_THREADS;   // >= RADIX: thread d < RADIX owns digit d in the scan phases
-constexpr int SORT_WARPS = SORT_THREADS / 32;
-constexpr int SORT_ITEMS = HCC_SORT_ITEMS;
-constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;   // 4096 pairs per CTA
+// Tile shape per key width (4096 pairs per CTA either way): 256 threads x 16 pairs for 32-bit
+// keys, 512 x 8 for 64-bit keys; launch bounds cap the registers (4 resp. 3 CTAs per SM)
+// because occupancy, not bandwidth, decides this kernel's speed.
+template <typename KeyT> struct SortCfg { static constexpr int THREADS = 256, ITEMS = 16, MIN_CTAS = 4; };
+template <> struct SortCfg<unsigned long long> { static constexpr int THREADS = 512, ITEMS = 8, MIN_CTAS = 3; };
+constexpr int SORT_TILE = 4096;
 constexpr int MAX_PASSES = 8;
 constexpr uint32_t FLAG_AGG = 1u << 30, FLAG_PREFIX = 2u << 30, VAL_MASK = (1u << 30) - 1u;
 constexpr int HIST_THREADS = 256;
-constexpr int SORT_MIN_CTAS = HCC_SORT_MIN_CTAS;  // caps the registers: occupancy decides this kernel's speed
+constexpr uint32_t FEW_DIGITS = 16;
 constexpr int LOOK = 4;                      // look-back rows fetched per round trip
 
 // control region of the workspace (zeroed once per sort by one memset)
 struct SortCtl {
     uint32_t hist[MAX_PASSES][RADIX];
     uint32_t ticket[MAX_PASSES];
-    uint32_t pad[8];
+    uint32_t few_digits[MAX_PASSES];   // pass p sees at most FEW_DIGITS distinct digit values
+
 };
 
 __device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t *p) {
@@ -65,7 +59,7 @@ k_histogram(const KeyT *__restrict__ keys, uint32_t n, uint32_t passes, SortCtl 
 // Exclusive scan of each digit histogram, written as the PREFIX row of "tile -1"
 // (row 0 of that pass's status array), so the look-back needs no special first tile.
 __global__ void __launch_bounds__(RADIX)
-k_scan_hist(const SortCtl *ctl, uint32_t *status, size_t status_stride) {
+k_scan_hist(SortCtl *ctl, uint32_t *status, size_t status_stride) {
     __shared__ uint32_t s_w[RADIX / 32];
     const uint32_t p = blockIdx.x, d = threadIdx.x, lane = d & 31u, warp = d >> 5;
     uint32_t v = ctl->hist[p][d], incl = v;
@@ -75,7 +69,8 @@ k_scan_hist(const SortCtl *ctl, uint32_t *status, size_t status_stride) {
         if (lane >= (uint32_t)o) incl += x;
     }
     if (lane == 31) s_w[warp] = incl;
-    __syncthreads();
+    const int distinct = __syncthreads_count(v != 0u);
+    if (d == 0) ctl->few_digits[p] = (uint32_t)distinct <= FEW_DIGITS ? 1u : 0u;
     uint32_t add = 0;
     for (uint32_t w = 0; w < warp; ++w) add += s_w[w];
     status[p * status_stride + d] = FLAG_PREFIX | (add + incl - v);
@@ -91,9 +86,12 @@ __global__ void k_iota(uint32_t *perm, uint32_t n) {
 // global base.  Tiles are handed out by an atomic ticket so that every predecessor of a
 // running tile is itself running or done (forward progress of the look-back spin).
 template <typename KeyT, bool FIRST, bool WRITE_KEYS>
-__global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_CTAS)
+__global__ void __launch_bounds__(SortCfg<KeyT>::THREADS, SortCfg<KeyT>::MIN_CTAS)
 k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const uint32_t *__restrict__ vals_in,
-           uint32_t *__restrict__ vals_out, uint32_t n, uint32_t shift, uint32_t *status, uint32_t *ticket) {
+           uint32_t *__restrict__ vals_out, uint32_t n, uint32_t shift, uint32_t *status, uint32_t *ticket,
+           const uint32_t *few_digits) {
+    constexpr int SORT_THREADS = SortCfg<KeyT>::THREADS, SORT_ITEMS = SortCfg<KeyT>::ITEMS, SORT_WARPS = SORT_THREADS / 32;
+    static_assert(SORT_THREADS * SORT_ITEMS == SORT_TILE && SORT_THREADS >= RADIX, "tile shape");
     __shared__ uint32_t s_warp_hist[SORT_WARPS][RADIX];
     __shared__ uint32_t s_tile_off[RADIX];
     __shared__ uint32_t s_gbase[RADIX];
@@ -108,6 +106,7 @@ k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const 
     for (uint32_t i = tid; i < SORT_WARPS * RADIX; i += SORT_THREADS) (&s_warp_hist[0][0])[i] = 0u;
     __syncthreads();
     const uint32_t tile = s_tile;
+    const bool use_match = *few_digits != 0u;      // uniform over the grid
     const uint32_t tile_base = tile * SORT_TILE;
     const uint32_t count = min((uint32_t)SORT_TILE, n - tile_base);
     const uint32_t my_base = warp * (SORT_ITEMS * 32) + lane;   // item i at my_base + 32*i (warp-striped)
@@ -125,14 +124,20 @@ k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const 
     for (int i = 0; i < SORT_ITEMS; ++i) {
         const bool valid = my_base + 32 * i < count;
         const uint32_t digit = valid ? ((uint32_t)(key[i] >> shift) & (RADIX - 1)) : (uint32_t)RADIX;
-        // lanes holding the same digit: one ballot per digit bit (MATCH.ANY costs a round per
-        // distinct value in the warp, far more on well-spread digits)
-        uint32_t peers = 0xFFFFFFFFu;
+        // lanes holding the same digit.  MATCH.ANY costs a round per distinct value in the warp:
+        // it wins when the pass has few distinct digits (hierarchy cut codes are like that), one
+        // ballot per digit bit wins on well-spread digits (TwoPoint's Morton codes)
+        uint32_t peers;
+        if (use_match) {
+            peers = __match_any_sync(0xFFFFFFFFu, digit);
+        } else {
+            peers = 0xFFFFFFFFu;
 #pragma unroll
-        for (int b = 0; b <= RADIX_BITS; ++b) {
-            const bool bit = (digit >> b) & 1u;
-            const uint32_t m = __ballot_sync(0xFFFFFFFFu, bit);
-            peers &= bit ? m : ~m;
+            for (int b = 0; b <= RADIX_BITS; ++b) {
+                const bool bit = (digit >> b) & 1u;
+                const uint32_t m = __ballot_sync(0xFFFFFFFFu, bit);
+                peers &= bit ? m : ~m;
+            }
         }
         const uint32_t below = __popc(peers & lt);
         const uint32_t old = s_warp_hist[warp][digit & (RADIX - 1)];
@@ -241,6 +246,7 @@ static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t *perm
     k_histogram<KeyT><<<hist_blocks, HIST_THREADS, 0, s>>>(keys, n, passes, ctl);
     k_scan_hist<<<passes, RADIX, 0, s>>>(ctl, status, status_stride);
     const size_t dyn = (sizeof(KeyT) + sizeof(uint32_t)) * SORT_TILE;
+    constexpr int SORT_THREADS = SortCfg<KeyT>::THREADS;
     static bool attr_done = false;
     if (!attr_done) {
         HCC_CUDA_TRY(cudaFuncSetAttribute(k_onesweep<KeyT, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
@@ -257,11 +263,12 @@ static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t *perm
         uint32_t *vin = ((passes - 1 - p) & 1u) ? perm : vals_tmp;
         uint32_t *st = status + (size_t)p * status_stride;
         uint32_t *tk = &ctl->ticket[p];
+        const uint32_t *fd = &ctl->few_digits[p];
         const uint32_t shift = RADIX_BITS * p;
-        if (first && last) k_onesweep<KeyT, true, false><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk);
-        else if (first)    k_onesweep<KeyT, true, true><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk);
-        else if (last)     k_onesweep<KeyT, false, false><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk);
-        else               k_onesweep<KeyT, false, true><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk);
+        if (first && last) k_onesweep<KeyT, true, false><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd);
+        else if (first)    k_onesweep<KeyT, true, true><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd);
+        else if (last)     k_onesweep<KeyT, false, false><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd);
+        else               k_onesweep<KeyT, false, true><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd);
         KeyT *t = kin; kin = kout; kout = t;
     }
     HCC_CUDA_TRY(cudaGetLastError());
