@@ -61,7 +61,7 @@ struct CutDev {
     uint32_t n_entries;                // sum over levels of n_tab*w
     uint32_t n_tables;
     uint32_t bits_used;
-    const float4 *boxes;               // 2 float4 per entry: (lo.xyz, cnt-of-table in entry 0), (hi.xyz, -)
+    const float4 *boxes;               // 2 float4 per entry: (lo.x, lo.y, hi.x, hi.y), (lo.z, hi.z, cnt-of-table in entry 0, -)
     const uint32_t *entry_node;
     const uint32_t *table_cnt;
 };

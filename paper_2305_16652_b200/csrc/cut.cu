@@ -98,8 +98,9 @@ k_build_tables(const hcc_node *__restrict__ nodes, const float *__restrict__ had
             uint32_t node = 0xFFFFFFFFu - (uint32_t)(ke & 0xFFFFFFFFull);
             hcc_node nd = nodes[node];
             ent[rank] = node;
-            box[2 * rank + 0] = make_float4(nd.lo[0], nd.lo[1], nd.lo[2], rank == 0 ? __uint_as_float(n_out) : 0.0f);
-            box[2 * rank + 1] = make_float4(nd.hi[0], nd.hi[1], nd.hi[2], 0.0f);
+            // entry layout for the encoder's packed arithmetic: {lo.x, lo.y | hi.x, hi.y}, {lo.z, hi.z | cnt, -}
+            box[2 * rank + 0] = make_float4(nd.lo[0], nd.lo[1], nd.hi[0], nd.hi[1]);
+            box[2 * rank + 1] = make_float4(nd.lo[2], nd.hi[2], rank == 0 ? __uint_as_float(n_out) : 0.0f, 0.0f);
         }
     }
     for (uint32_t j = n_out + lane; j < w; j += 32) {   // empty slots (and empty tables: cnt = 0 in slot 0)

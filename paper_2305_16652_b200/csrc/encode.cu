@@ -23,54 +23,88 @@ __device__ __forceinline__ float4 ld_stream(const float4 *p) {
     return r;
 }
 
+// Packed fp32 pairs (sm_100a add/mul.f32x2): two IEEE operations per issue slot, same rounding as
+// the scalar forms, so the slab arithmetic below is still the operation sequence hcc.h states.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float &lo, float &hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
 struct RayEnc {
-    float ox, oy, oz, tmin, ix, iy, iz, tmax;
+    f32x2 oxy, ozz, ixy, izz;   // (o.x, o.y), (o.z, o.z), (1/d.x, 1/d.y), (1/d.z, 1/d.z)
+    float tmin, tmax;
 };
 
+// Cut box entry in memory (cut.cu): A = {lo.x, lo.y | hi.x, hi.y}, B = {lo.z, hi.z | cnt, -}.
 // Alg. 1 line 5: t1 = (lo - o) * inv, t2 = (hi - o) * inv per axis (subtract, round, multiply,
 // round), tn = max(tmin, max_a min(t1,t2)), tf = min(tmax, min_a max(t1,t2)), hit <=> tn <= tf.
 // min/max drop NaN operands, so the reduction order does not matter.
-__device__ __forceinline__ bool slab_hit(const RayEnc &r, const float4 lo, const float4 hi) {
-    float t1x = (lo.x - r.ox) * r.ix, t2x = (hi.x - r.ox) * r.ix;
-    float t1y = (lo.y - r.oy) * r.iy, t2y = (hi.y - r.oy) * r.iy;
-    float t1z = (lo.z - r.oz) * r.iz, t2z = (hi.z - r.oz) * r.iz;
+__device__ __forceinline__ bool slab_hit(const RayEnc &r, const ulonglong2 A, const f32x2 Bz) {
+    float t1x, t1y, t2x, t2y, t1z, t2z;
+    unpack2(mul2(sub2(A.x, r.oxy), r.ixy), t1x, t1y);
+    unpack2(mul2(sub2(A.y, r.oxy), r.ixy), t2x, t2y);
+    unpack2(mul2(sub2(Bz, r.ozz), r.izz), t1z, t2z);
     float tn = fmaxf(max3(fminf(t1x, t2x), fminf(t1y, t2y), fminf(t1z, t2z)), r.tmin);
     float tf = fminf(min3(fmaxf(t1x, t2x), fmaxf(t1y, t2y), fmaxf(t1z, t2z)), r.tmax);
     return tn <= tf;
 }
 
+__device__ __forceinline__ ulonglong2 ldg_u2(const ulonglong2 *p) {
+    ulonglong2 r;
+    asm volatile("ld.global.nc.v2.u64 {%0,%1}, [%2];" : "=l"(r.x), "=l"(r.y) : "l"(p));
+    return r;
+}
+
 // Mask of one table over entries [j0, j1): entry j -> bit (j1-1-j) of the result (<= 32 entries).
 template <bool SMEM>
-__device__ __forceinline__ uint32_t table_mask(const RayEnc &r, const float4 *__restrict__ box, uint32_t j0, uint32_t j1) {
+__device__ __forceinline__ uint32_t table_mask(const RayEnc &r, const ulonglong2 *__restrict__ box, uint32_t j0, uint32_t j1) {
     uint32_t mask = 0;
 #pragma unroll 4
     for (uint32_t j = j0; j < j1; ++j) {
-        float4 lo, hi;
-        if (SMEM) { lo = box[2 * j]; hi = box[2 * j + 1]; }
-        else      { lo = __ldg(box + 2 * j); hi = __ldg(box + 2 * j + 1); }
-        mask = (mask << 1) | (slab_hit(r, lo, hi) ? 1u : 0u);
+        ulonglong2 A, B;
+        if (SMEM) { A = box[2 * j]; B = box[2 * j + 1]; }
+        else      { A = ldg_u2(box + 2 * j); B = ldg_u2(box + 2 * j + 1); }
+        mask = (mask << 1) | (slab_hit(r, A, B.x) ? 1u : 0u);
     }
     return mask;
 }
 
 constexpr int ENC_THREADS = 256;
+constexpr int ENC_THREADS_MAX = 1024;   // one big CTA per SM when the staged tables leave room for only one
 
 // Alg. 1: line 1 "copy cut nodes from global memory into shared memory" (the first
 // smem_entries entries = whole levels), line 2 grid-stride "while have ray", lines 4-6 per
 // level.  One ray per thread per iteration; 32-byte rays read as two 16-byte loads.
 template <typename KeyT>
-__global__ void __launch_bounds__(ENC_THREADS)
+__global__ void __launch_bounds__(ENC_THREADS_MAX)
 k_encode_hcc(const float4 *__restrict__ rays, uint64_t n, const CutDev cut, uint32_t smem_entries,
              KeyT *__restrict__ keys) {
-    extern __shared__ float4 s_box[];
-    for (uint32_t i = threadIdx.x; i < 2u * smem_entries; i += ENC_THREADS) s_box[i] = cut.boxes[i];
+    extern __shared__ ulonglong2 s_box[];
+    const ulonglong2 *g_box = reinterpret_cast<const ulonglong2 *>(cut.boxes);
+    for (uint32_t i = threadIdx.x; i < 2u * smem_entries; i += blockDim.x) s_box[i] = g_box[i];
     __syncthreads();
-    const uint64_t stride = (uint64_t)gridDim.x * ENC_THREADS;
-    for (uint64_t ri = (uint64_t)blockIdx.x * ENC_THREADS + threadIdx.x; ri < n; ri += stride) {
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t ri = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; ri < n; ri += stride) {
         float4 a = ld_stream(rays + 2 * ri), b = ld_stream(rays + 2 * ri + 1);
         RayEnc r;
-        r.ox = a.x; r.oy = a.y; r.oz = a.z; r.tmin = a.w;
-        r.ix = 1.0f / b.x; r.iy = 1.0f / b.y; r.iz = 1.0f / b.z; r.tmax = b.w;
+        const float iz = 1.0f / b.z;
+        r.oxy = pack2(a.x, a.y); r.ozz = pack2(a.z, a.z); r.tmin = a.w;
+        r.ixy = pack2(1.0f / b.x, 1.0f / b.y); r.izz = pack2(iz, iz); r.tmax = b.w;
         unsigned long long key = 0;
         uint32_t table = 0;
         bool alive = true;
@@ -80,8 +114,8 @@ k_encode_hcc(const float4 *__restrict__ rays, uint64_t n, const CutDev cut, uint
             if (alive) {
                 const uint32_t e0 = cut.ent_off[l] + table * w;
                 const bool in_smem = e0 < smem_entries;           // uniform per level
-                const float4 *box = in_smem ? s_box + 2 * (size_t)e0 : cut.boxes + 2 * (size_t)e0;
-                const uint32_t cnt = __float_as_uint(in_smem ? box[0].w : __ldg(&box[0].w));
+                const ulonglong2 *box = in_smem ? s_box + 2 * (size_t)e0 : g_box + 2 * (size_t)e0;
+                const uint32_t cnt = (uint32_t)(in_smem ? box[1].y : ldg_u2(box + 1).y);   // low word = count
                 // entries [0,cnt) are valid; entry j -> bit (w-1-j)
                 uint32_t c_hi = cnt > 32u ? cnt - 32u : 0u;       // only flat tables wider than 32
                 unsigned long long m_hi = 0;
@@ -133,10 +167,10 @@ k_encode_twopoint(const float4 *__restrict__ rays, uint64_t n, float3 lo, float3
     }
 }
 
-static int grid_for(const void *kernel, size_t smem, uint64_t n) {
+static int grid_for(const void *kernel, size_t smem, uint64_t n, int threads = ENC_THREADS) {
     int per_sm = 1;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, ENC_THREADS, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
-    uint64_t want = (n + ENC_THREADS - 1) / ENC_THREADS;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+    uint64_t want = (n + threads - 1) / threads;
     uint64_t cap = (uint64_t)sm_count() * (uint64_t)per_sm;
     return (int)(want < cap ? want : cap);
 }
@@ -162,14 +196,16 @@ extern "C" int32_t hcc_encode(const float *rays_dev, uint64_t n, const hcc_cut *
         if ((size_t)end * 32 <= budget) smem_entries = end; else break;
     }
     size_t smem = (size_t)smem_entries * 32;
+    // CTA size: as many resident threads per SM as the staged tables allow
+    const int threads = smem > 100 * 1024 ? 1024 : smem > 48 * 1024 ? 512 : ENC_THREADS;
     if (cut->container_bits == 32) {
         auto kern = k_encode_hcc<uint32_t>;
         HCC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget));
-        kern<<<grid_for((const void *)kern, smem, n), ENC_THREADS, smem, s>>>((const float4 *)rays_dev, n, d, smem_entries, (uint32_t *)keys_dev);
+        kern<<<grid_for((const void *)kern, smem, n, threads), threads, smem, s>>>((const float4 *)rays_dev, n, d, smem_entries, (uint32_t *)keys_dev);
     } else {
         auto kern = k_encode_hcc<unsigned long long>;
         HCC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget));
-        kern<<<grid_for((const void *)kern, smem, n), ENC_THREADS, smem, s>>>((const float4 *)rays_dev, n, d, smem_entries, (unsigned long long *)keys_dev);
+        kern<<<grid_for((const void *)kern, smem, n, threads), threads, smem, s>>>((const float4 *)rays_dev, n, d, smem_entries, (unsigned long long *)keys_dev);
     }
     HCC_CUDA_TRY(cudaGetLastError());
     return HCC_OK;
