@@ -185,6 +185,33 @@ HCC_API int32_t hcc_encode(const float *rays_dev, uint64_t n, const hcc_cut *cut
 HCC_API int32_t hcc_encode_twopoint(const float *rays_dev, uint64_t n, const float scene_lo[3],
                             const float scene_hi[3], uint32_t key_bits, void *keys_dev, void *stream);
 
+/* ---- NEXT rows of the scope table -------------------------------------------
+ * (f3) Prefix path code, PAPER.md:116-128 (section 4.1, Figure 5): "setting each bit to 1 if the
+ * corresponding node intersection result is true, and 0 otherwise ... when the rays are forced
+ * to traverse the BVH in the same order", the walk ended after key_bits tests.  The walk: depth
+ * first, left child before right, starting with the root's own test; every node visited gets the
+ * slab test of hcc_encode on the ray's [tmin, tmax] and contributes one bit, the first test in
+ * bit key_bits-1; a hit internal node has its children visited next, a hit leaf nothing more (no
+ * triangle tests); an exhausted walk leaves the remaining low bits zero.  The paper's upper-bound
+ * ordering, not a practical one (:128).  keys_dev: uint32[n] if key_bits <= 32 else uint64[n]. */
+HCC_API int32_t hcc_encode_ppc(const hcc_bvh *bvh, const float *rays_dev, uint64_t n, uint32_t key_bits,
+                       void *keys_dev, void *stream);
+
+/* (f4) Regular grid encoding: "the BVH cut nodes are replaced by grids that divide
+ * the space evenly".  Fills `cut` with level tables of the given widths (powers of two >= 2, sum
+ * <= key_bits) whose entries are cells of a regular subdivision of the root box, so hcc_encode
+ * and the rest of the path run unchanged.  A cell is named by its path of halvings; halving i
+ * (counted from the root, across levels) splits axis i mod 3, bit 0 = lower half; entry j of a
+ * table is the cell whose path bits of that level are j (first halving in the top bit).  With
+ * n_a halvings of axis a and cell index i_a:  lo_a = scene_lo_a + (scene_hi_a - scene_lo_a) *
+ * (i_a / 2^n_a) (fp32, three operations), hi_a likewise at i_a + 1, exactly scene_hi_a for the
+ * last cell.  All tables are full; hcc_cut_read returns HCC_INVALID_NODE for every entry. */
+HCC_API int32_t hcc_select_grid(const hcc_bvh *bvh, const uint32_t *widths, uint32_t m, uint32_t key_bits,
+                        hcc_cut *cut, void *stream);
+
+/* Boxes of all table entries of `cut` as 6 floats (lo.xyz, hi.xyz) each, in entry order (host). */
+HCC_API int32_t hcc_cut_read_boxes(const hcc_cut *cut, float *boxes_host, void *stream);
+
 /* ---- (a3) sort ------------------------------------------------------------------------
  * Stable ascending order of ray ids by key ("sorting the HCCs as natural
  * numbers", :247 "sorts the indices of rays"): perm_dev[j] = id of the ray at rank j; equal
@@ -195,6 +222,15 @@ HCC_API int32_t hcc_encode_twopoint(const float *rays_dev, uint64_t n, const flo
 HCC_API int32_t hcc_sort_workspace_bytes(uint64_t n, uint32_t container_bits, uint64_t *bytes);
 HCC_API int32_t hcc_sort(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bits_used,
                  uint32_t *perm_dev, void *workspace_dev, uint64_t workspace_bytes, void *stream);
+
+/* Sort-cost reduction the paper proposes (§6.6.1 "skip the last few bits during
+ * encoding and terminate bucket sorting early"): the stable ascending order by the key bits
+ * [bit_lo, bit_hi) only, i.e. by (key >> bit_lo); bits at and above bit_hi must be zero.  Rays
+ * whose keys differ only below bit_lo keep their input order.  ceil((bit_hi - bit_lo) / 8) radix
+ * passes.  hcc_sort(.., bits_used, ..) == hcc_sort_range(.., 0, bits_used, ..).  Other arguments,
+ * workspace and errors as hcc_sort. */
+HCC_API int32_t hcc_sort_range(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bit_lo, uint32_t bit_hi,
+                       uint32_t *perm_dev, void *workspace_dev, uint64_t workspace_bytes, void *stream);
 
 /* ---- (a4) trace -----------------------------------------------------------------------
  * Rays are traced in the order perm_dev[0], perm_dev[1], ... (perm_dev == NULL: 0, 1, ...,
@@ -223,6 +259,9 @@ HCC_API int32_t hcc_trace_stats(const hcc_bvh *bvh, const float *rays_dev, uint6
 HCC_API int32_t hcc_pipeline_create(uint64_t n_max, uint32_t container_bits_max, uint32_t host_staging,
                             hcc_pipeline **out);
 HCC_API int32_t hcc_pipeline_destroy(hcc_pipeline *p);
+/* Low key bits the pipeline's sort leaves unordered (hcc_sort_range's bit_lo);
+ * 0 = the full sort (default).  Values above the key's used bits mean "do not sort at all". */
+HCC_API int32_t hcc_pipeline_set_sort_skip_bits(hcc_pipeline *p, uint32_t bits);
 
 /* Enqueue encode + sort + trace of one batch on `stream` (device pointers).
  *  order HCC_ORDER_HCC:      keys = hcc_encode(rays, cut);               `cut` required

@@ -39,6 +39,14 @@ def _load():
         L.oracle_encode_hcc.restype = None
         L.oracle_encode_twopoint.argtypes = [_vp, _u64, _vp, _vp, _u32, _vp]
         L.oracle_encode_twopoint.restype = None
+        L.oracle_grid_tables.argtypes = [_vp, _vp, _vp, _u32, _vp]
+        L.oracle_grid_tables.restype = None
+        L.oracle_encode_tables.argtypes = [_vp, _u64, _vp, _vp, _u32, _vp, _vp]
+        L.oracle_encode_tables.restype = None
+        L.oracle_encode_ppc.argtypes = [_vp, _u64, _vp, _u32, _vp]
+        L.oracle_encode_ppc.restype = ctypes.c_int
+        L.oracle_sort_from_bit.argtypes = [_vp, _u64, _u32, _vp]
+        L.oracle_sort_from_bit.restype = ctypes.c_int
         L.oracle_sort.argtypes = [_vp, _u64, _vp]
         L.oracle_sort.restype = ctypes.c_int
         L.oracle_tri_hit.argtypes = [_vp, _vp, _vp]
@@ -203,12 +211,55 @@ def encode_twopoint(rays, scene_lo, scene_hi, key_bits):
     return keys
 
 
+def grid_tables(scene_lo, scene_hi, widths):
+    """(f4, reading R14) boxes [n_entries, 6] of the regular-grid level tables and
+    the per-table counts (all full)."""
+    lo = _c(scene_lo, np.float32); hi = _c(scene_hi, np.float32)
+    w = np.asarray(widths, dtype=np.uint32)
+    n_ent = n_tab = 0
+    nt = 1
+    for x in w:
+        n_ent += nt * int(x); n_tab += nt; nt *= int(x)
+    boxes = np.empty((n_ent, 6), dtype=np.float32)
+    _load().oracle_grid_tables(lo.ctypes.data, hi.ctypes.data, w.ctypes.data, len(w), boxes.ctypes.data)
+    cnt = np.concatenate([np.full(int(np.prod(w[:l], dtype=np.int64)), int(w[l]), dtype=np.uint32) for l in range(len(w))])
+    return boxes, cnt
+
+
+def encode_tables(rays, boxes, widths, table_cnt):
+    """The multi-level code over explicit boxes (regular grid, f4); uint64 [n]."""
+    rays = _rays(rays); boxes = _c(boxes, np.float32); table_cnt = _c(table_cnt, np.uint32)
+    w = np.asarray(widths, dtype=np.uint32)
+    keys = np.empty(rays.shape[0], dtype=np.uint64)
+    _load().oracle_encode_tables(rays.ctypes.data, rays.shape[0], boxes.ctypes.data, w.ctypes.data, len(w),
+                                 table_cnt.ctypes.data, keys.ctypes.data)
+    return keys
+
+
+def encode_ppc(rays, nodes, bits):
+    """(f3, reading R13) prefix path code; uint64 [n]."""
+    rays = _rays(rays); nodes = _c(nodes)
+    keys = np.empty(rays.shape[0], dtype=np.uint64)
+    if _load().oracle_encode_ppc(rays.ctypes.data, rays.shape[0], nodes.ctypes.data, int(bits), keys.ctypes.data) != 0:
+        raise RuntimeError("oracle_encode_ppc: stack overflow")
+    return keys
+
+
 # --------------------------------------------------------------------------- (a3)
 def sort(keys):
     """Stable ascending permutation of ray ids by key; uint32 [n]."""
     keys = _c(keys, np.uint64)
     perm = np.empty(keys.shape[0], dtype=np.uint32)
     if _load().oracle_sort(keys.ctypes.data, keys.shape[0], perm.ctypes.data) != 0:
+        raise MemoryError
+    return perm
+
+
+def sort_from_bit(keys, bit_lo):
+    """(f1) stable ascending permutation by the keys without their low bit_lo bits."""
+    keys = _c(keys, np.uint64)
+    perm = np.empty(keys.shape[0], dtype=np.uint32)
+    if _load().oracle_sort_from_bit(keys.ctypes.data, keys.shape[0], int(bit_lo), perm.ctypes.data) != 0:
         raise MemoryError
     return perm
 

@@ -252,6 +252,114 @@ void oracle_encode_hcc(const float *rays, uint64_t n_rays, const node_t *nodes,
     }
 }
 
+/* (f4) Regular grid encoding — PAPER.md:243: "the BVH cut nodes are replaced by grids that
+ * divide the space evenly".  Reading R14 (the paper gives no layout): the level tables of the
+ * hierarchy cut code are kept (widths w[0..m-1], powers of two) and every table entry is a
+ * cell of a regular subdivision of the scene box: a cell is named by its path of halvings,
+ * halving i (counted from the root, across levels) splits axis i mod 3, bit 0 = lower half;
+ * entry j of a table is the cell whose log2(w) path bits of that level are j (first halving
+ * in the most significant bit).  With n_a halvings of axis a so far and cell index i_a:
+ *   lo_a = scene_lo_a + (scene_hi_a - scene_lo_a) * (i_a / 2^n_a)        (three fp32 operations)
+ *   hi_a = the same at i_a + 1, and exactly scene_hi_a for the last cell.
+ * boxes: 6 floats (lo, hi) per entry, tables laid out like oracle_level_tables. */
+void oracle_grid_tables(const float *scene_lo, const float *scene_hi, const uint32_t *w, uint32_t m, float *boxes) {
+    size_t ent_off = 0, n_tables = 1;
+    uint32_t halvings = 0;
+    for (uint32_t l = 0; l < m; ++l) {
+        uint32_t k = 0;
+        while ((1u << k) < w[l]) ++k;
+        for (size_t t = 0; t < n_tables; ++t) {
+            for (uint32_t j = 0; j < w[l]; ++j) {
+                /* path of the cell: the table's path (t, halvings bits) followed by j (k bits) */
+                uint64_t path = ((uint64_t)t << k) | j;
+                uint32_t total = halvings + k;
+                uint32_t idx[3] = {0, 0, 0}, cnt[3] = {0, 0, 0};
+                for (uint32_t i = 0; i < total; ++i) {
+                    uint32_t bit = (uint32_t)(path >> (total - 1 - i)) & 1u;
+                    idx[i % 3] = (idx[i % 3] << 1) | bit;
+                    cnt[i % 3] += 1;
+                }
+                float *b = boxes + 6 * (ent_off + t * w[l] + j);
+                for (int a = 0; a < 3; ++a) {
+                    float ext = scene_hi[a] - scene_lo[a];
+                    float cells = (float)(1u << cnt[a]);
+                    b[a] = scene_lo[a] + ext * ((float)idx[a] / cells);
+                    b[3 + a] = idx[a] + 1u == (1u << cnt[a]) ? scene_hi[a] : scene_lo[a] + ext * ((float)(idx[a] + 1u) / cells);
+                }
+            }
+        }
+        ent_off += n_tables * w[l];
+        n_tables *= w[l];
+        halvings += k;
+    }
+}
+
+/* The multi-level code of oracle_encode_hcc over explicit boxes (6 floats per entry) instead of
+ * BVH nodes: same levels, same bit layout R9, same representative rule. */
+void oracle_encode_tables(const float *rays, uint64_t n_rays, const float *boxes, const uint32_t *w, uint32_t m,
+                          const uint32_t *table_cnt, uint64_t *keys) {
+    for (uint64_t r = 0; r < n_rays; ++r) {
+        const float *ray = rays + 8 * r;
+        uint64_t key = 0;
+        size_t ent_off = 0, tab_off = 0, n_tables = 1, table = 0;
+        int alive = 1;
+        for (uint32_t l = 0; l < m; ++l) {
+            uint64_t mask = 0;
+            int rep = -1;
+            if (alive) {
+                uint32_t c = table_cnt[tab_off + table];
+                const float *b = boxes + 6 * (ent_off + table * w[l]);
+                for (uint32_t j = 0; j < c; ++j) {
+                    if (slab_hit(ray, b + 6 * j, b + 6 * j + 3)) {
+                        mask |= (uint64_t)1 << (w[l] - 1 - j);
+                        if (rep < 0) rep = (int)j;
+                    }
+                }
+            }
+            key = (key << w[l]) | mask;
+            if (rep < 0) alive = 0; else table = table * w[l] + (size_t)rep;
+            ent_off += n_tables * w[l];
+            tab_off += n_tables;
+            n_tables *= w[l];
+        }
+        keys[r] = key;
+    }
+}
+
+/* (f3) Prefix path code — PAPER.md:116-128 (section 4.1, Figure 5): "the prefix path code is formed
+ * by setting each bit to 1 if the corresponding node intersection result is true, and 0
+ * otherwise ... when the rays are forced to traverse the BVH in the same order", the traversal
+ * "terminat[ed] ... after a certain number of bits have been set".  Reading R13: depth-first,
+ * left child before right child, starting with the root's own test; every node popped is
+ * tested (slab test R7 on the ray's [tmin, tmax]) and contributes one bit, first test in the
+ * most significant of the `bits` bits; a hit internal node pushes its children, a hit leaf
+ * does nothing more (no triangle tests); the walk stops after `bits` tests or when the stack
+ * is empty (remaining low bits zero).  Returns -1 if the fixed stack overflowed. */
+int oracle_encode_ppc(const float *rays, uint64_t n_rays, const node_t *nodes, uint32_t bits, uint64_t *keys) {
+    enum { PPC_STACK = 128 };
+    for (uint64_t r = 0; r < n_rays; ++r) {
+        const float *ray = rays + 8 * r;
+        uint32_t stack[PPC_STACK];
+        int sp = 0;
+        uint64_t key = 0;
+        uint32_t done = 0;
+        stack[sp++] = 0;
+        while (sp > 0 && done < bits) {
+            const node_t *nd = &nodes[stack[--sp]];
+            int hit = slab_hit(ray, nd->lo, nd->hi);
+            key = (key << 1) | (uint64_t)hit;
+            ++done;
+            if (hit && nd->count == 0) {
+                if (sp + 2 > PPC_STACK) return -1;
+                stack[sp++] = nd->left_or_first + 1; /* right: visited after the whole left subtree */
+                stack[sp++] = nd->left_or_first;
+            }
+        }
+        keys[r] = done < bits ? key << (bits - done) : key;
+    }
+    return 0;
+}
+
 /* TwoPoint (details R10): origin and the estimated termination
  * point o + (0.25*e)*d (e = largest extent of the scene box, d unit) are quantised to
  * b = floor(B/6) bits per coordinate inside the scene box and bit-interleaved in the order
@@ -318,6 +426,19 @@ int oracle_sort(const uint64_t *keys, uint64_t n, uint32_t *perm) {
     merge_sort(k, perm, tk, tv, 0, n);
     free(k); free(tk); free(tv);
     return 0;
+}
+
+/* (f1) Sort truncation — PAPER.md:428 (section 6.6.1): "skip the last few bits during encoding
+ * and terminate bucket sorting early".  Reading: the order is the stable ascending order of the
+ * keys with their low bit_lo bits dropped, so rays whose codes differ only in those bits keep
+ * their input order.  Written out as that definition: shift, then the same stable sort. */
+int oracle_sort_from_bit(const uint64_t *keys, uint64_t n, uint32_t bit_lo, uint32_t *perm) {
+    uint64_t *k = (uint64_t *)malloc(sizeof(uint64_t) * (n ? n : 1));
+    if (!k) return -1;
+    for (uint64_t i = 0; i < n; ++i) k[i] = bit_lo >= 64 ? 0 : keys[i] >> bit_lo;
+    int rc = oracle_sort(k, n, perm);
+    free(k);
+    return rc;
 }
 
 /* ------------------------------------------------------------------------- */

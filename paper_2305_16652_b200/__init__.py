@@ -42,6 +42,11 @@ _SIGNATURES = {
     "hcc_encode_twopoint": [_vp, _u64, _vp, _vp, _u32, _vp, _vp],
     "hcc_sort_workspace_bytes": [_u64, _u32, _pu64],
     "hcc_sort": [_vp, _u64, _u32, _u32, _vp, _vp, _u64, _vp],
+    "hcc_encode_ppc": [_vp, _vp, _u64, _u32, _vp, _vp],
+    "hcc_select_grid": [_vp, _vp, _u32, _u32, _vp, _vp],
+    "hcc_cut_read_boxes": [_vp, _vp, _vp],
+    "hcc_sort_range": [_vp, _u64, _u32, _u32, _u32, _vp, _vp, _u64, _vp],
+    "hcc_pipeline_set_sort_skip_bits": [_vp, _u32],
     "hcc_trace": [_vp, _vp, _u64, _vp, _i32, _vp, _vp],
     "hcc_pipeline_create": [_u64, _u32, _u32, ctypes.POINTER(_vp)],
     "hcc_pipeline_destroy": [_vp],
@@ -175,6 +180,12 @@ class Cut:
         _check(lib().hcc_cut_read(self._h, ent.ctypes.data, cnt.ctypes.data, _stream(stream)))
         return ent, cnt
 
+    def read_boxes(self, stream=None):
+        """hcc_cut_read_boxes: float32 [n_entries, 6] (lo.xyz, hi.xyz) on the host."""
+        boxes = np.empty((self.info()["n_entries"], 6), dtype=np.float32)
+        _check(lib().hcc_cut_read_boxes(self._h, boxes.ctypes.data, _stream(stream)))
+        return boxes
+
     def close(self):
         if getattr(self, "_h", None) is not None and self._h:
             lib().hcc_cut_destroy(self._h)
@@ -198,6 +209,15 @@ def select_cut_levels(bvh, density_dev, widths, key_bits, cut=None, stream=None)
         cut = Cut(max(int(np.prod(w.astype(np.int64))), 64))
     _check(lib().hcc_select_cut_levels(bvh._h, _dev(density_dev, (torch.float32,), "density"), w.ctypes.data,
                                        w.shape[0], int(key_bits), cut._h, _stream(stream)))
+    return cut
+
+
+def select_grid(bvh, widths, key_bits, cut=None, stream=None):
+    """hcc_select_grid (f4): level tables whose entries are regular grid cells."""
+    w = np.ascontiguousarray(widths, dtype=np.uint32)
+    if cut is None:
+        cut = Cut(max(int(np.prod(w.astype(np.int64))), 64))
+    _check(lib().hcc_select_grid(bvh._h, w.ctypes.data, w.shape[0], int(key_bits), cut._h, _stream(stream)))
     return cut
 
 
@@ -249,6 +269,16 @@ def encode_twopoint(rays, scene_lo, scene_hi, key_bits, keys=None, stream=None):
     return keys
 
 
+def encode_ppc(bvh, rays, key_bits, keys=None, stream=None):
+    """hcc_encode_ppc (f3): prefix path code of every ray."""
+    n = rays.shape[0]
+    dt = _key_dtype(32 if key_bits <= 32 else 64)
+    if keys is None:
+        keys = torch.empty(n, dtype=dt, device="cuda")
+    _check(lib().hcc_encode_ppc(bvh._h, _rays_dev(rays), n, int(key_bits), _dev(keys, (dt,), "keys"), _stream(stream)))
+    return keys
+
+
 # ---------------------------------------------------------------------------------- (a3)
 def sort_workspace_bytes(n, container_bits):
     need = _u64()
@@ -256,17 +286,18 @@ def sort_workspace_bytes(n, container_bits):
     return int(need.value)
 
 
-def sort(keys, bits_used, perm=None, workspace=None, stream=None):
-    """hcc_sort: stable ascending permutation of ray ids (int32 CUDA [n]).  keys is clobbered."""
+def sort(keys, bits_used, perm=None, workspace=None, stream=None, bit_lo=0):
+    """hcc_sort / hcc_sort_range: stable ascending permutation of ray ids (int32 CUDA [n]) by the key
+    bits [bit_lo, bits_used).  keys is clobbered."""
     n = keys.shape[0]
     cb = 32 if keys.dtype == torch.int32 else 64
     if perm is None:
         perm = torch.empty(n, dtype=torch.int32, device="cuda")
     if workspace is None:
         workspace = torch.empty(sort_workspace_bytes(n, cb), dtype=torch.uint8, device="cuda")
-    _check(lib().hcc_sort(_dev(keys, (torch.int32, torch.int64), "keys"), n, cb, int(bits_used),
-                          _dev(perm, (torch.int32,), "perm"), _vp(workspace.data_ptr()), workspace.numel(),
-                          _stream(stream)))
+    _check(lib().hcc_sort_range(_dev(keys, (torch.int32, torch.int64), "keys"), n, cb, int(bit_lo), int(bits_used),
+                                _dev(perm, (torch.int32,), "perm"), _vp(workspace.data_ptr()), workspace.numel(),
+                                _stream(stream)))
     return perm
 
 
@@ -329,6 +360,10 @@ class Pipeline:
         self.n_max = int(n_max)
         _check(lib().hcc_pipeline_create(self.n_max, int(container_bits_max), 1 if host_staging else 0,
                                          ctypes.byref(self._h)))
+
+    def set_sort_skip_bits(self, bits):
+        """hcc_pipeline_set_sort_skip_bits: low key bits the sort leaves unordered."""
+        _check(lib().hcc_pipeline_set_sort_skip_bits(self._h, int(bits)))
 
     def reorder_trace(self, bvh, cut, order, rays, mode=TRACE_CLOSEST, hits=None, key_bits=32,
                       perm_out=None, stream=None):

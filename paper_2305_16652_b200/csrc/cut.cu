@@ -3,6 +3,8 @@
 // rule that maps a (K, key_bits) request onto the paper's encoders (R-ML).
 #include <string.h>
 
+#include <vector>
+
 #include "common.cuh"
 
 namespace hcc {
@@ -179,12 +181,10 @@ extern "C" int32_t hcc_cut_destroy(hcc_cut *c) {
 
 static bool key_bits_ok(uint32_t b) { return b == 16 || b == 24 || b == 32 || b == 48 || b == 64; }
 
-extern "C" int32_t hcc_select_cut_levels(const hcc_bvh *bvh, const float *density_dev, const uint32_t *widths,
-                                         uint32_t m, uint32_t key_bits, hcc_cut *cut, void *stream) {
-    HCC_REQUIRE(bvh && density_dev && widths && cut, HCC_ERR_INVALID_ARG, "hcc_select_cut: NULL argument");
+// Lays the level tables of widths[0..m-1] out in the handle's buffers (no kernel runs).
+static int32_t set_levels(hcc_cut *cut, const uint32_t *widths, uint32_t m, uint32_t key_bits) {
     HCC_REQUIRE(key_bits_ok(key_bits), HCC_ERR_INVALID_ARG, "hcc_select_cut: key_bits must be 16, 24, 32, 48 or 64");
     HCC_REQUIRE(m >= 1 && m <= HCC_MAX_LEVELS, HCC_ERR_INVALID_ARG, "hcc_select_cut: 1..%u levels", HCC_MAX_LEVELS);
-    HCC_REQUIRE(aligned(density_dev, 16), HCC_ERR_BAD_ALIGNMENT, "hcc_select_cut: density_dev not 16-byte aligned");
     CutDev d;
     memset(&d, 0, sizeof d);
     d.m = m;
@@ -216,7 +216,88 @@ extern "C" int32_t hcc_select_cut_levels(const hcc_bvh *bvh, const float *densit
     cut->container_bits = key_bits <= 32 ? 32u : 64u;
     cut->K_eff = (uint32_t)(nt);
     cut->valid = true;
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_select_cut_levels(const hcc_bvh *bvh, const float *density_dev, const uint32_t *widths,
+                                         uint32_t m, uint32_t key_bits, hcc_cut *cut, void *stream) {
+    HCC_REQUIRE(bvh && density_dev && widths && cut, HCC_ERR_INVALID_ARG, "hcc_select_cut: NULL argument");
+    HCC_REQUIRE(aligned(density_dev, 16), HCC_ERR_BAD_ALIGNMENT, "hcc_select_cut: density_dev not 16-byte aligned");
+    int32_t rc = set_levels(cut, widths, m, key_bits);
+    if (rc != HCC_OK) return rc;
     return launch_build_tables(bvh, density_dev, cut, (cudaStream_t)stream);
+}
+
+// (f4) regular grid tables; the cell rule is stated in include/hcc.h
+__global__ void k_build_grid(CutDev d, uint32_t level, uint32_t halvings_before, uint32_t k, float3 lo, float3 hi,
+                             uint32_t *__restrict__ entry_node, uint32_t *__restrict__ table_cnt, float4 *__restrict__ boxes) {
+    const uint32_t w = d.w[level];
+    const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;        // entry within the level
+    if (e >= d.n_tab[level] * w) return;
+    const uint32_t t = e / w, j = e % w;
+    const unsigned long long path = ((unsigned long long)t << k) | j;
+    const uint32_t total = halvings_before + k;
+    uint32_t idx[3] = {0u, 0u, 0u}, cnt[3] = {0u, 0u, 0u};
+    for (uint32_t i = 0; i < total; ++i) {
+        const uint32_t bit = (uint32_t)(path >> (total - 1u - i)) & 1u;
+        idx[i % 3u] = (idx[i % 3u] << 1) | bit;
+        cnt[i % 3u] += 1u;
+    }
+    const float slo[3] = {lo.x, lo.y, lo.z}, shi[3] = {hi.x, hi.y, hi.z};
+    float blo[3], bhi[3];
+    for (int a = 0; a < 3; ++a) {
+        const float ext = shi[a] - slo[a];
+        const float cells = (float)(1u << cnt[a]);
+        blo[a] = slo[a] + ext * ((float)idx[a] / cells);
+        bhi[a] = idx[a] + 1u == (1u << cnt[a]) ? shi[a] : slo[a] + ext * ((float)(idx[a] + 1u) / cells);
+    }
+    const size_t o = d.ent_off[level] + e;
+    entry_node[o] = HCC_INVALID_NODE;
+    boxes[2 * o + 0] = make_float4(blo[0], blo[1], bhi[0], bhi[1]);
+    boxes[2 * o + 1] = make_float4(blo[2], bhi[2], j == 0 ? __uint_as_float(w) : 0.0f, 0.0f);
+    if (j == 0) table_cnt[d.tab_off[level] + t] = w;
+}
+
+extern "C" int32_t hcc_select_grid(const hcc_bvh *bvh, const uint32_t *widths, uint32_t m, uint32_t key_bits,
+                                   hcc_cut *cut, void *stream) {
+    HCC_REQUIRE(bvh && widths && cut, HCC_ERR_INVALID_ARG, "hcc_select_grid: NULL argument");
+    uint32_t halvings = 0, ks[HCC_MAX_LEVELS];
+    for (uint32_t l = 0; l < m && l < HCC_MAX_LEVELS; ++l) {
+        HCC_REQUIRE(widths[l] >= 2 && (widths[l] & (widths[l] - 1u)) == 0u, HCC_ERR_INVALID_ARG,
+                    "hcc_select_grid: level widths must be powers of two >= 2");
+        ks[l] = 31u - (uint32_t)__builtin_clz(widths[l]);
+        halvings += ks[l];
+    }
+    HCC_REQUIRE(halvings <= 60u, HCC_ERR_UNSUPPORTED, "hcc_select_grid: more than 60 halvings");
+    int32_t rc = set_levels(cut, widths, m, key_bits);
+    if (rc != HCC_OK) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    const float3 lo = make_float3(bvh->scene_lo[0], bvh->scene_lo[1], bvh->scene_lo[2]);
+    const float3 hi = make_float3(bvh->scene_hi[0], bvh->scene_hi[1], bvh->scene_hi[2]);
+    uint32_t before = 0;
+    for (uint32_t l = 0; l < m; ++l) {
+        const uint32_t n = cut->dev.n_tab[l] * cut->dev.w[l];
+        k_build_grid<<<(n + 255u) / 256u, 256, 0, s>>>(cut->dev, l, before, ks[l], lo, hi, cut->d_entry_node, cut->d_table_cnt, cut->d_boxes);
+        before += ks[l];
+    }
+    HCC_CUDA_TRY(cudaGetLastError());
+    return HCC_OK;
+}
+
+// Boxes of all table entries as 6 floats (lo, hi) each, in entry order (tests, diagnostics).
+extern "C" int32_t hcc_cut_read_boxes(const hcc_cut *cut, float *boxes_host, void *stream) {
+    HCC_REQUIRE(cut && cut->valid && boxes_host, HCC_ERR_INVALID_ARG, "hcc_cut_read_boxes: bad argument");
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t n = cut->dev.n_entries;
+    std::vector<float> raw(8 * n);
+    HCC_CUDA_TRY(cudaMemcpyAsync(raw.data(), cut->d_boxes, sizeof(float) * 8 * n, cudaMemcpyDeviceToHost, s));
+    HCC_CUDA_TRY(cudaStreamSynchronize(s));
+    for (size_t e = 0; e < n; ++e) {
+        const float *r = raw.data() + 8 * e;   // {lo.x, lo.y, hi.x, hi.y}, {lo.z, hi.z, cnt, -}
+        float *o = boxes_host + 6 * e;
+        o[0] = r[0]; o[1] = r[1]; o[2] = r[4]; o[3] = r[2]; o[4] = r[3]; o[5] = r[5];
+    }
+    return HCC_OK;
 }
 
 extern "C" int32_t hcc_select_cut(const hcc_bvh *bvh, const float *density_dev, uint32_t K, uint32_t key_bits,

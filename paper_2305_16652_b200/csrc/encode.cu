@@ -167,6 +167,44 @@ k_encode_twopoint(const float4 *__restrict__ rays, uint64_t n, float3 lo, float3
     }
 }
 
+// (f3) prefix path code, PAPER.md:116-128 (Figure 5); the walk is stated in include/hcc.h.
+// One ray per thread, depth-first with the left child first over the canonical fp32 nodes; each
+// popped node's slab test (the same arithmetic as slab_hit above) appends one bit.
+constexpr int PPC_STACK = 66;   // depth <= 63 (hcc_bvh_create): at most depth + 1 pending nodes
+template <typename KeyT>
+__global__ void __launch_bounds__(ENC_THREADS)
+k_encode_ppc(const float4 *__restrict__ rays, uint64_t n, const float4 *__restrict__ nodes, uint32_t bits,
+             KeyT *__restrict__ keys) {
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t ri = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; ri < n; ri += stride) {
+        float4 a = ld_stream(rays + 2 * ri), b = ld_stream(rays + 2 * ri + 1);
+        RayEnc r;
+        const float iz = 1.0f / b.z;
+        r.oxy = pack2(a.x, a.y); r.ozz = pack2(a.z, a.z); r.tmin = a.w;
+        r.ixy = pack2(1.0f / b.x, 1.0f / b.y); r.izz = pack2(iz, iz); r.tmax = b.w;
+        uint32_t stack[PPC_STACK];
+        int sp = 0;
+        unsigned long long key = 0;
+        uint32_t done = 0;
+        stack[sp++] = 0u;
+        while (sp > 0 && done < bits) {
+            const uint32_t i = stack[--sp];
+            const float4 n0 = __ldg(nodes + 2 * (size_t)i), n1 = __ldg(nodes + 2 * (size_t)i + 1);   // lo.xyz hi.x | hi.yz left count
+            ulonglong2 A;
+            A.x = pack2(n0.x, n0.y); A.y = pack2(n0.w, n1.x);
+            const bool hit = slab_hit(r, A, pack2(n0.z, n1.y));
+            key = (key << 1) | (hit ? 1ull : 0ull);
+            ++done;
+            if (hit && __float_as_uint(n1.w) == 0u) {
+                const uint32_t left = __float_as_uint(n1.z);
+                stack[sp++] = left + 1u;
+                stack[sp++] = left;
+            }
+        }
+        keys[ri] = (KeyT)(done < bits ? key << (bits - done) : key);
+    }
+}
+
 static int grid_for(const void *kernel, size_t smem, uint64_t n, int threads = ENC_THREADS) {
     int per_sm = 1;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
@@ -231,6 +269,29 @@ extern "C" int32_t hcc_encode_twopoint(const float *rays_dev, uint64_t n, const 
     } else {
         auto kern = k_encode_twopoint<unsigned long long>;
         kern<<<grid_for((const void *)kern, 0, n), ENC_THREADS, 0, s>>>((const float4 *)rays_dev, n, lo, hi, len, b, (unsigned long long *)keys_dev);
+    }
+    HCC_CUDA_TRY(cudaGetLastError());
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_encode_ppc(const hcc_bvh *bvh, const float *rays_dev, uint64_t n, uint32_t key_bits, void *keys_dev,
+                                  void *stream) {
+    HCC_REQUIRE(bvh, HCC_ERR_INVALID_ARG, "hcc_encode_ppc: NULL bvh");
+    HCC_REQUIRE(key_bits == 16 || key_bits == 24 || key_bits == 32 || key_bits == 48 || key_bits == 64,
+                HCC_ERR_INVALID_ARG, "hcc_encode_ppc: key_bits must be 16, 24, 32, 48 or 64");
+    if (n == 0) return HCC_OK;
+    HCC_REQUIRE(rays_dev && keys_dev, HCC_ERR_INVALID_ARG, "hcc_encode_ppc: NULL argument");
+    HCC_REQUIRE(aligned(rays_dev, 32) && aligned(keys_dev, 16), HCC_ERR_BAD_ALIGNMENT,
+                "hcc_encode_ppc: rays need 32-byte, keys 16-byte alignment");
+    HCC_REQUIRE(n < (1ull << 32), HCC_ERR_UNSUPPORTED, "hcc_encode_ppc: n >= 2^32");
+    cudaStream_t s = (cudaStream_t)stream;
+    const float4 *nodes = reinterpret_cast<const float4 *>(bvh->d_nodes);
+    if (key_bits <= 32) {
+        auto kern = k_encode_ppc<uint32_t>;
+        kern<<<grid_for((const void *)kern, 0, n), ENC_THREADS, 0, s>>>((const float4 *)rays_dev, n, nodes, key_bits, (uint32_t *)keys_dev);
+    } else {
+        auto kern = k_encode_ppc<unsigned long long>;
+        kern<<<grid_for((const void *)kern, 0, n), ENC_THREADS, 0, s>>>((const float4 *)rays_dev, n, nodes, key_bits, (unsigned long long *)keys_dev);
     }
     HCC_CUDA_TRY(cudaGetLastError());
     return HCC_OK;

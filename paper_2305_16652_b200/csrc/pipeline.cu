@@ -19,6 +19,7 @@ struct hcc_pipeline {
     void *d_hits;       // host-buffer form only
     cudaEvent_t ev[6];  // h2d start, encode start, sort start, trace start, trace end, d2h end
     bool timed, timed_host;
+    uint32_t sort_skip_bits;   // low key bits the sort leaves unordered (hcc_sort_range)
 };
 
 namespace hcc {
@@ -88,6 +89,13 @@ extern "C" int32_t hcc_pipeline_create(uint64_t n_max, uint32_t container_bits_m
     return HCC_OK;
 }
 
+extern "C" int32_t hcc_pipeline_set_sort_skip_bits(hcc_pipeline *p, uint32_t bits) {
+    HCC_REQUIRE(p, HCC_ERR_INVALID_ARG, "hcc_pipeline_set_sort_skip_bits: NULL pipeline");
+    HCC_REQUIRE(bits <= 64, HCC_ERR_INVALID_ARG, "hcc_pipeline_set_sort_skip_bits: bits > 64");
+    p->sort_skip_bits = bits;
+    return HCC_OK;
+}
+
 extern "C" int32_t hcc_reorder_trace(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
                                      uint32_t key_bits, const float *rays_dev, uint64_t n, int32_t mode,
                                      void *hits_dev, uint32_t *perm_out_dev, void *stream) {
@@ -116,7 +124,8 @@ extern "C" int32_t hcc_reorder_trace(hcc_pipeline *p, const hcc_bvh *bvh, const 
     if (rc != HCC_OK) return rc;
     HCC_CUDA_TRY(cudaEventRecord(p->ev[2], s));
     if (order != HCC_ORDER_NOSORT) {
-        rc = hcc_sort(p->d_keys, n, container, bits_used, perm, p->d_ws, p->ws_bytes, stream);
+        const uint32_t lo = p->sort_skip_bits < bits_used ? p->sort_skip_bits : bits_used;
+        rc = hcc_sort_range(p->d_keys, n, container, lo, bits_used, perm, p->d_ws, p->ws_bytes, stream);
         if (rc != HCC_OK) return rc;
     }
     HCC_CUDA_TRY(cudaEventRecord(p->ev[3], s));

@@ -40,14 +40,14 @@ __device__ __forceinline__ void st_volatile_u32(uint32_t *p, uint32_t v) {
 // All digit histograms in one read of the keys.
 template <typename KeyT>
 __global__ void __launch_bounds__(HIST_THREADS)
-k_histogram(const KeyT *__restrict__ keys, uint32_t n, uint32_t passes, SortCtl *ctl) {
+k_histogram(const KeyT *__restrict__ keys, uint32_t n, uint32_t passes, uint32_t bit_lo, SortCtl *ctl) {
     __shared__ uint32_t sh[MAX_PASSES][RADIX];
     for (uint32_t i = threadIdx.x; i < MAX_PASSES * RADIX; i += HIST_THREADS) (&sh[0][0])[i] = 0u;
     __syncthreads();
     const uint32_t stride = gridDim.x * HIST_THREADS;
     for (uint32_t i = blockIdx.x * HIST_THREADS + threadIdx.x; i < n; i += stride) {
         KeyT k = keys[i];
-        for (uint32_t p = 0; p < passes; ++p) atomicAdd(&sh[p][(uint32_t)(k >> (RADIX_BITS * p)) & (RADIX - 1)], 1u);
+        for (uint32_t p = 0; p < passes; ++p) atomicAdd(&sh[p][(uint32_t)(k >> (bit_lo + RADIX_BITS * p)) & (RADIX - 1)], 1u);
     }
     __syncthreads();
     for (uint32_t i = threadIdx.x; i < passes * RADIX; i += HIST_THREADS) {
@@ -231,7 +231,7 @@ static uint64_t ctl_bytes(uint64_t n) {
 }
 
 template <typename KeyT>
-static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t *perm, unsigned char *ws, cudaStream_t s) {
+static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t bit_lo, uint32_t *perm, unsigned char *ws, cudaStream_t s) {
     const uint32_t tiles = (n + SORT_TILE - 1) / SORT_TILE;
     KeyT *keys_tmp = reinterpret_cast<KeyT *>(ws);
     uint32_t *vals_tmp = reinterpret_cast<uint32_t *>(ws + round_up(sizeof(KeyT) * (uint64_t)n, 256));
@@ -243,7 +243,7 @@ static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t *perm
     int hist_blocks = (int)((n + HIST_THREADS * 16 - 1) / (HIST_THREADS * 16));
     int cap = sm_count() * 4;
     if (hist_blocks > cap) hist_blocks = cap;
-    k_histogram<KeyT><<<hist_blocks, HIST_THREADS, 0, s>>>(keys, n, passes, ctl);
+    k_histogram<KeyT><<<hist_blocks, HIST_THREADS, 0, s>>>(keys, n, passes, bit_lo, ctl);
     k_scan_hist<<<passes, RADIX, 0, s>>>(ctl, status, status_stride);
     const size_t dyn = (sizeof(KeyT) + sizeof(uint32_t)) * SORT_TILE;
     constexpr int SORT_THREADS = SortCfg<KeyT>::THREADS;
@@ -264,7 +264,7 @@ static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t *perm
         uint32_t *st = status + (size_t)p * status_stride;
         uint32_t *tk = &ctl->ticket[p];
         const uint32_t *fd = &ctl->few_digits[p];
-        const uint32_t shift = RADIX_BITS * p;
+        const uint32_t shift = bit_lo + RADIX_BITS * p;
         if (first && last) k_onesweep<KeyT, true, false><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd);
         else if (first)    k_onesweep<KeyT, true, true><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd);
         else if (last)     k_onesweep<KeyT, false, false><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd);
@@ -287,10 +287,10 @@ extern "C" int32_t hcc_sort_workspace_bytes(uint64_t n, uint32_t container_bits,
     return HCC_OK;
 }
 
-extern "C" int32_t hcc_sort(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bits_used, uint32_t *perm_dev,
-                            void *workspace_dev, uint64_t workspace_bytes, void *stream) {
+extern "C" int32_t hcc_sort_range(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bit_lo, uint32_t bit_hi,
+                                  uint32_t *perm_dev, void *workspace_dev, uint64_t workspace_bytes, void *stream) {
     HCC_REQUIRE(container_bits == 32 || container_bits == 64, HCC_ERR_INVALID_ARG, "hcc_sort: container_bits must be 32 or 64");
-    HCC_REQUIRE(bits_used <= container_bits, HCC_ERR_INVALID_ARG, "hcc_sort: bits_used > container_bits");
+    HCC_REQUIRE(bit_lo <= bit_hi && bit_hi <= container_bits, HCC_ERR_INVALID_ARG, "hcc_sort: need bit_lo <= bit_hi <= container_bits");
     HCC_REQUIRE(n < (1ull << 30), HCC_ERR_UNSUPPORTED, "hcc_sort: n >= 2^30");
     if (n == 0) return HCC_OK;
     HCC_REQUIRE(keys_dev && perm_dev && workspace_dev, HCC_ERR_INVALID_ARG, "hcc_sort: NULL argument");
@@ -301,13 +301,19 @@ extern "C" int32_t hcc_sort(void *keys_dev, uint64_t n, uint32_t container_bits,
     HCC_REQUIRE(workspace_bytes >= need, HCC_ERR_INVALID_ARG, "hcc_sort: workspace too small (%llu < %llu)",
                 (unsigned long long)workspace_bytes, (unsigned long long)need);
     cudaStream_t s = (cudaStream_t)stream;
-    const uint32_t passes = (bits_used + RADIX_BITS - 1) / RADIX_BITS;
+    const uint32_t passes = (bit_hi - bit_lo + RADIX_BITS - 1) / RADIX_BITS;
     if (passes == 0) {
         k_iota<<<(uint32_t)((n + 255) / 256), 256, 0, s>>>(perm_dev, (uint32_t)n);
         HCC_CUDA_TRY(cudaGetLastError());
         return HCC_OK;
     }
     unsigned char *ws = reinterpret_cast<unsigned char *>(round_up(reinterpret_cast<uintptr_t>(workspace_dev), 256));
-    if (container_bits == 32) return sort_impl<uint32_t>((uint32_t *)keys_dev, (uint32_t)n, passes, perm_dev, ws, s);
-    return sort_impl<unsigned long long>((unsigned long long *)keys_dev, (uint32_t)n, passes, perm_dev, ws, s);
+    if (container_bits == 32) return sort_impl<uint32_t>((uint32_t *)keys_dev, (uint32_t)n, passes, bit_lo, perm_dev, ws, s);
+    return sort_impl<unsigned long long>((unsigned long long *)keys_dev, (uint32_t)n, passes, bit_lo, perm_dev, ws, s);
+}
+
+extern "C" int32_t hcc_sort(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bits_used, uint32_t *perm_dev,
+                            void *workspace_dev, uint64_t workspace_bytes, void *stream) {
+    HCC_REQUIRE(bits_used <= container_bits, HCC_ERR_INVALID_ARG, "hcc_sort: bits_used > container_bits");
+    return hcc_sort_range(keys_dev, n, container_bits, 0u, bits_used, perm_dev, workspace_dev, workspace_bytes, stream);
 }

@@ -1,0 +1,185 @@
+"""Pins of the oracle functions behind the NEXT rows of the scope table:
+f1 sort truncation, f3 prefix path code (Figure 5),
+f4 regular grid encoding.  CPU only."""
+import os
+
+import numpy as np
+import pytest
+
+import hcc_inputs
+import oracle
+from hcc_inputs import rng as hrng
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _rays(n, seed, lo=-0.1, hi=1.1):
+    u = hrng.u01(seed, 0, np.arange(n, dtype=np.uint64), np.arange(6, dtype=np.uint64)[:, None]).T
+    r = np.zeros((n, 8), dtype=np.float32)
+    r[:, 0:3] = lo + (hi - lo) * u[:, 0:3]
+    d = 2.0 * u[:, 3:6] - 1.0
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    r[:, 4:7] = d
+    r[:, 7] = np.inf
+    return r
+
+
+# ------------------------------------------------------------------------------- f1
+@pytest.mark.parametrize("bit_lo", [0, 1, 7, 8, 13, 16, 31, 32, 40, 64])
+def test_sort_from_bit_is_the_stable_sort_of_the_shifted_keys(bit_lo):
+    n = 5000
+    keys = hrng.hash_u64(0xF1, 0, np.arange(n, dtype=np.uint64), 0) >> np.uint64(16)      # 48-bit keys
+    keys[::3] = keys[1::3][: keys[::3].shape[0]]                                        # duplicates
+    want = np.argsort(keys >> np.uint64(bit_lo) if bit_lo < 64 else np.zeros_like(keys), kind="stable").astype(np.uint32)
+    got = oracle.sort_from_bit(keys, bit_lo)
+    assert np.array_equal(got, want)
+    if bit_lo == 0:
+        assert np.array_equal(got, oracle.sort(keys))
+    if bit_lo >= 48:                       # nothing left to order by: the input order
+        assert np.array_equal(got, np.arange(n, dtype=np.uint32))
+
+
+def test_sort_from_bit_keeps_input_order_below_the_cut():
+    """Keys that differ only below bit_lo keep their input order (the arrangement
+    of rays inside a bucket does not matter)."""
+    hi = np.repeat(np.arange(7, dtype=np.uint64)[::-1], 50) << np.uint64(8)
+    lo = hrng.hash_u64(3, 0, np.arange(hi.shape[0], dtype=np.uint64), 0) & np.uint64(0xFF)
+    perm = oracle.sort_from_bit(hi | lo, 8)
+    for v in range(7):
+        ids = perm[(hi[perm] >> np.uint64(8)) == v]
+        assert np.all(np.diff(ids.astype(np.int64)) > 0)
+    assert np.all(np.diff((hi[perm] >> np.uint64(8)).astype(np.int64)) >= 0)
+
+
+# ------------------------------------------------------------------------------- f4
+@pytest.mark.parametrize("widths", [[8], [16, 8], [4, 4, 4], [2, 16], [16, 16, 16]])
+def test_grid_cells_partition_their_parent(widths):
+    lo, hi = np.array([-1.0, 0.5, 2.0], np.float32), np.array([3.0, 1.5, 2.75], np.float32)
+    boxes, cnt = oracle.grid_tables(lo, hi, widths)
+    assert np.all(cnt == np.concatenate([np.full(int(np.prod(widths[:l])), widths[l]) for l in range(len(widths))]))
+    b = boxes.astype(np.float64)
+    assert np.all(b[:, 3:6] > b[:, 0:3])
+    vol = np.prod(b[:, 3:6] - b[:, 0:3], axis=1)
+    off, nt, parent_vol = 0, 1, np.array([np.prod(hi.astype(np.float64) - lo.astype(np.float64))])
+    for w in widths:
+        v = vol[off:off + nt * w].reshape(nt, w)
+        assert np.allclose(v.sum(axis=1), parent_vol, rtol=1e-5)       # the cells of a table tile its parent cell
+        assert np.allclose(v, parent_vol[:, None] / w, rtol=1e-5)      # "divide the space evenly"
+        tb = b[off:off + nt * w].reshape(nt, w, 6)
+        if off:   # inside the parent cell
+            pb = b[poff:poff + nt].reshape(nt, 1, 6)
+            assert np.all(tb[:, :, 0:3] >= pb[:, :, 0:3] - 1e-6) and np.all(tb[:, :, 3:6] <= pb[:, :, 3:6] + 1e-6)
+        else:     # the first level spans exactly the scene box
+            assert np.array_equal(boxes[:w, 0:3].min(axis=0), lo) and np.array_equal(boxes[:w, 3:6].max(axis=0), hi)
+        parent_vol, poff = v.reshape(-1), off
+        off += nt * w
+        nt *= w
+
+
+def test_grid_halving_order_and_entry_index():
+    """Halving i splits axis i mod 3 with bit 0 = lower half; entry j = the path bits, first
+    halving on top (reading R14): for one level of 8 cells, entry j = 4*ix + 2*iy + iz."""
+    boxes, _ = oracle.grid_tables([0, 0, 0], [1, 1, 1], [8])
+    for j in range(8):
+        ix, iy, iz = (j >> 2) & 1, (j >> 1) & 1, j & 1
+        assert np.array_equal(boxes[j], np.array([ix, iy, iz, ix + 1, iy + 1, iz + 1], np.float32) * 0.5)
+    # a fourth halving returns to x: 16 cells = 4 x 2 x 2
+    boxes, _ = oracle.grid_tables([0, 0, 0], [1, 1, 1], [16])
+    assert np.array_equal(np.unique(boxes[:, 0]), np.array([0, 0.25, 0.5, 0.75], np.float32))
+    assert np.array_equal(np.unique(boxes[:, 1]), np.array([0, 0.5], np.float32))
+
+
+def test_grid_keys_mark_the_cells_a_ray_crosses():
+    """Closed form: a ray along +x through the middle of a row of a 4x2x2 grid crosses the 4
+    cells of that row, in a one-level code those are exactly the set bits; the bit of the cell
+    holding the origin is always set (origin inside a box => hit)."""
+    w = [16]
+    boxes, cnt = oracle.grid_tables([0, 0, 0], [1, 1, 1], w)
+    ray = np.array([[-1.0, 0.25, 0.75, 0.0, 1.0, 0.0, 0.0, np.inf]], np.float32)
+    key = int(oracle.encode_tables(ray, boxes, w, cnt)[0])
+    want = 0
+    for j in range(16):                       # path bits x y z x: ix = (b3 b0), iy = b2, iz = b1
+        iy, iz = (j >> 2) & 1, (j >> 1) & 1
+        if iy == 0 and iz == 1:
+            want |= 1 << (15 - j)
+    assert key == want and bin(key).count("1") == 4
+    rays = _rays(2000, 0x6A1D, lo=0.01, hi=0.99)
+    keys = oracle.encode_tables(rays, boxes, w, cnt)
+    cell = np.floor(rays[:, 0:3].astype(np.float64) * np.array([4, 2, 2])).astype(np.int64)
+    j = ((cell[:, 0] >> 1) << 3) | (cell[:, 1] << 2) | (cell[:, 2] << 1) | (cell[:, 0] & 1)
+    assert np.all((keys >> (15 - j).astype(np.uint64)) & np.uint64(1) == 1)
+
+
+def test_encode_tables_agrees_with_encode_hcc_on_node_boxes(tiny):
+    """The generic table encoder fed the cut's own node boxes is the hierarchy cut code."""
+    b = tiny.bvh
+    for K, bits in ((32, 32), (64, 32), (256, 32)):
+        tables, _, _ = oracle.select_cut(b.nodes, K, bits)
+        ent = tables.entry_node.astype(np.int64)
+        ent[tables.entry_node == 0xFFFFFFFF] = 0
+        boxes = np.concatenate([b.nodes["lo"][ent], b.nodes["hi"][ent]], axis=1).astype(np.float32)
+        want = oracle.encode_hcc(tiny.diffuse, b.nodes, tables)
+        got = oracle.encode_tables(tiny.diffuse, boxes, tables.widths, tables.table_cnt)
+        assert np.array_equal(got, want)
+
+
+# ------------------------------------------------------------------------------- f3
+def _fig5_tree():
+    """Root with two children; the left child has two leaf children (Figure 5)."""
+    tri = lambda x, y: [[x, y, 0.5], [x + 0.1, y, 0.5], [x, y + 0.1, 0.5]]
+    tris = np.array([tri(0.1, 0.1), tri(0.1, 0.7), tri(0.7, 0.4)], np.float32)
+    nodes = [((0, 0, 0.4), (1, 1, 0.6), 1, 0),          # 0 root
+             ((0, 0, 0.4), (0.3, 1, 0.6), 3, 0),        # 1 left, internal
+             ((0.6, 0.3, 0.4), (0.9, 0.6, 0.6), 2, 1),  # 2 right, leaf
+             ((0, 0, 0.4), (0.3, 0.3, 0.6), 0, 1),      # 3 leaf
+             ((0, 0.6, 0.4), (0.3, 1, 0.6), 1, 1)]      # 4 leaf
+    return hcc_inputs.make_bvh(nodes, tris)
+
+
+def test_ppc_figure5_golden():
+    """PAPER.md:120, Figure 5: "the first four intersection results of the rays are true, true,
+    false, and false, resulting in a 4-bit prefix code of 1100"."""
+    with open(os.path.join(GOLDEN, "fig5_ppc.txt")) as f:
+        want = [ln.split()[0] for ln in f if ln.strip() and not ln.startswith("#")][0]
+    b = _fig5_tree()
+    # crosses the root and the left child's box between its two leaf boxes (y = 0.45), in -z
+    ray = np.array([[0.15, 0.45, 2.0, 0.0, 0.0, 0.0, -1.0, np.inf]], np.float32)
+    assert format(int(oracle.encode_ppc(ray, b.nodes, 4)[0]), "04b") == want == "1100"
+    # order of visits: root, left, left.left, left.right, right  -> 5th bit is the right child's test
+    assert format(int(oracle.encode_ppc(ray, b.nodes, 16)[0]), "016b") == "11000" + "0" * 11
+    hit_right = np.array([[0.75, 0.45, 2.0, 0.0, 0.0, 0.0, -1.0, np.inf]], np.float32)
+    assert format(int(oracle.encode_ppc(hit_right, b.nodes, 16)[0]), "016b") == "101" + "0" * 13   # left missed: its subtree is skipped
+    miss = np.array([[5.0, 5.0, 2.0, 0.0, 0.0, 0.0, -1.0, np.inf]], np.float32)
+    assert int(oracle.encode_ppc(miss, b.nodes, 16)[0]) == 0
+
+
+def _ppc_recursive(ray, nodes, bits):
+    """Independent statement of the walk: recursive pre-order, one oracle.slab_hit per visit."""
+    out = []
+
+    def visit(i):
+        if len(out) >= bits:
+            return
+        hit = oracle.slab_hit(ray, nodes["lo"][i], nodes["hi"][i])
+        out.append(1 if hit else 0)
+        if hit and nodes["count"][i] == 0:
+            l = int(nodes["left_or_first"][i])
+            visit(l)
+            visit(l + 1)
+    visit(0)
+    out += [0] * (bits - len(out))
+    return int("".join(map(str, out)), 2)
+
+
+@pytest.mark.parametrize("bits", [16, 32, 64])
+def test_ppc_vs_recursive_walk_and_prefix_property(tiny, bits):
+    b = tiny.bvh
+    rays = np.concatenate([tiny.diffuse[:150], tiny.shadow[:150], _rays(100, 0x99C, lo=-0.5, hi=1.5)])
+    keys = oracle.encode_ppc(rays, b.nodes, bits)
+    for i in range(rays.shape[0]):
+        assert int(keys[i]) == _ppc_recursive(rays[i], b.nodes, bits)
+    if bits > 16:   # a shorter code is the prefix of a longer one ("prefix path code")
+        assert np.array_equal(oracle.encode_ppc(rays, b.nodes, 16), keys >> np.uint64(bits - 16))
+    root_hit = np.array([oracle.slab_hit(r, b.nodes["lo"][0], b.nodes["hi"][0]) for r in rays])
+    assert np.array_equal((keys >> np.uint64(bits - 1)).astype(bool), root_hit)
+    assert np.all(keys[~root_hit] == 0)
