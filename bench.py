@@ -42,6 +42,9 @@ UNIT = "Mrays/s"
 #          2 compares: both quantised child boxes, trace.cu) + 36 per triangle test (the formula in
 #          include/hcc.h); encode: 26 per exact fp32 slab test (6 sub, 6 mul, 12 min/max, compare, bit).
 OPS_BOX, OPS_PAIR, OPS_TRI = 26, 34, 36
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the two trace kernels on config 2, from the
+# ncu --set full capture summarised in profiles/r1b_ncu_full.md (a profiler number, config "room" only)
+NCU_TRAFFIC_ROOM = {"diffuse": 41.129472e6 + 0.702976e6, "shadow": 79.268864e6 + 4.357632e6}
 SM_COUNT, LANES_PER_SM = 148, 128
 
 
@@ -354,7 +357,10 @@ def run_ours(args):
                ("diffuse", "encode"), ("shadow", "encode")), key=lambda k: orders["hcc"][k[0]][k[1] + "_ms"])
     roof = dict(stages[dom[0]][dom[1]])
     roof = {"bound": roof["bound"], "achieved": roof["achieved"], "peak": roof["peak"], "unit": roof["unit"],
-            "frac": roof["frac"], "traffic": None, "kernel": f"{dom[1]} ({dom[0]} batch)",
+            "frac": roof["frac"],
+            "traffic": NCU_TRAFFIC_ROOM[dom[0]] if (args.workload == "room" and dom[1] == "trace" and args.bounce == 1 and args.res_scale == 1.0) else None,
+            "traffic_unit": "bytes per launch (dram read + write, ncu, profiles/r1b_ncu_full.md)",
+            "kernel": f"{dom[1]} ({dom[0]} batch)",
             "peak_source": (f"{peak_kind} HBM copy" if roof["bound"] == "hbm" else
                             f"148 SMs x 128 fp32 lanes x {sm_max_mhz:.0f} MHz (DESIGN.md)")}
 
@@ -400,6 +406,64 @@ def run_ours(args):
                                      "unit": "GB/s", "frac": nb * (32 + tkb) / tp_ms / 1e6 / hbm_gbs}}
         del big, keys_b, keys_b0, ws_b, perm_b, tp_keys
         torch.cuda.empty_cache()
+
+    # ---- studies, on request: f1 sort truncation, f2 lambda and
+    #      ANC, f3 prefix path code (:116-128), f4 regular grid (:243)
+    studies = None
+    if args.studies and world == 1:
+        def med_ms(fn, setup=None, k=5):
+            out = []
+            for i in range(k + 1):
+                if setup:
+                    setup()
+                flush.zero_()
+                s0, e0 = ev(), ev()
+                s0.record(); fn(); e0.record()
+                torch.cuda.synchronize()
+                if i >= 1:
+                    out.append(s0.elapsed_time(e0))
+            return float(np.median(out))
+
+        def run_order(make_keys, bits_used, bit_lo=0):
+            """encode / sort / trace medians and ANC per batch for one key function (None = NoSort)."""
+            res = {}
+            for rays, mode, name in batches:
+                nb = rays.shape[0]
+                if make_keys is None:
+                    tr = med_ms(lambda: hcc.trace(bvh, rays, None, mode, hits=hits[name]))
+                    res[name] = {"encode_ms": 0.0, "sort_ms": 0.0, "trace_ms": tr, "mrays_per_s_incl": nb / tr / 1e3,
+                                 "mrays_per_s_trace_only": nb / tr / 1e3}
+                    continue
+                keys = make_keys(rays)
+                keys0 = keys.clone()
+                cb = 32 if keys.dtype == torch.int32 else 64
+                ws = torch.empty(hcc.sort_workspace_bytes(nb, cb), dtype=torch.uint8, device="cuda")
+                perm = torch.empty(nb, dtype=torch.int32, device="cuda")
+                enc = med_ms(lambda: make_keys(rays, keys))
+                srt = med_ms(lambda: hcc.sort(keys, bits_used, perm=perm, workspace=ws, bit_lo=bit_lo), setup=lambda: keys.copy_(keys0))
+                tr = med_ms(lambda: hcc.trace(bvh, rays, perm, mode, hits=hits[name]))
+                res[name] = {"encode_ms": enc, "sort_ms": srt, "trace_ms": tr, "mrays_per_s_incl": nb / (enc + srt + tr) / 1e3,
+                             "mrays_per_s_trace_only": nb / tr / 1e3, "anc": hcc.anc(keys0, perm)}
+            return res
+
+        hcc_keys = lambda cut_: (lambda rays, keys=None: hcc.encode(rays, cut_, keys=keys))
+        studies = {"truncation": {}, "lambda": {}, "orders": {}}
+        for skip in (0, 8, 16, 24, info["bits_used"]):
+            if skip <= info["bits_used"]:
+                studies["truncation"][f"skip_{skip}_bits"] = run_order(hcc_keys(cut), info["bits_used"], bit_lo=skip)
+        for lam in (0.1, 0.125, 0.25, 0.5, 1.0):
+            cut_l = hcc.select_cut(bvh, hcc.density(bvh, lam), w.K, w.key_bits)
+            studies["lambda"][f"{lam}"] = run_order(hcc_keys(cut_l), cut_l.info()["bits_used"])
+        grid_cut = hcc.select_grid(bvh, info["widths"], w.key_bits)
+        tp_bits = 6 * (w.key_bits // 6)
+        studies["orders"] = {
+            "nosort": run_order(None, 0),
+            "twopoint": run_order(lambda rays, keys=None: hcc.encode_twopoint(rays, bvh.scene_lo, bvh.scene_hi, w.key_bits, keys=keys), tp_bits),
+            "hcc": run_order(hcc_keys(cut), info["bits_used"]),
+            "grid": run_order(hcc_keys(grid_cut), info["bits_used"]),
+            "ppc": run_order(lambda rays, keys=None: hcc.encode_ppc(bvh, rays, w.key_bits, keys=keys), w.key_bits)}
+        studies["note"] = ("per batch medians of 5; grid = regular-grid tables of the same widths through the same encoder; "
+                           "ppc = prefix path code with key_bits tests (upper-bound ordering, PAPER.md:128)")
 
     # ---- e2e: the same step through the C ABI with HOST buffers (pinned), copies inside the timing
     rays_pin = {"diffuse": torch.from_numpy(diffuse_h).pin_memory(), "shadow": torch.from_numpy(shadow_h).pin_memory()}
@@ -461,7 +525,7 @@ def run_ours(args):
             "roofline": roof, "cpu_baseline": cpu,
             "cut": {"widths": info["widths"], "K_eff": info["K_eff"], "bits_used": info["bits_used"],
                     "container_bits": container, "cut_ms": cut_ms},
-            "orders": orders, "speedup_hcc": speed, "stages_roofline_hcc": stages, "stages_roofline_large_batch": large,
+            "orders": orders, "speedup_hcc": speed, "stages_roofline_hcc": stages, "stages_roofline_large_batch": large, "studies": studies,
             "diagnostics": diag,
             "paper_context": "RTX 3060, Breakfast: HCC 67.6 vs NoSort 37.4 vs TwoPoint 56.8 Mrays/s trace-only (PAPER.md:294-299); not comparable"}
     print(json.dumps(line))
@@ -482,6 +546,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--bounce", type=int, default=1, help="which bounce's ray batches to run (1 = rays off the primary hits)")
     ap.add_argument("--res-scale", type=float, default=1.0, help="image scale of the workload (1.0 = the config's resolution)")
+    ap.add_argument("--studies", action="store_true", help="add the NEXT-row studies: sort truncation, lambda/ANC, grid and PPC orders")
     ap.add_argument("--no-large-n", action="store_true", help="skip the large-batch encode/sort roofline leg")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
