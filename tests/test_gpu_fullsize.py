@@ -1,0 +1,96 @@
+"""Parity at BASELINE.json's full sizes, through the call bench.py times (hcc_reorder_trace on whole
+batches): config 2 in full (1,048,576 + 2,097,152 rays) and config 3 in full (16.6 M + 33.2 M rays).
+The oracle cannot run these batches whole, so: keys and hits of a seeded SAMPLE of rays are compared
+with the oracle one by one (bit-exact keys, hits within the north_star's bars), and the permutation
+is checked by the properties that define it at any size (a permutation; keys non-decreasing along
+it; equal keys in ascending ray id = stability).  The primaries that spawn the batches are traced by
+the library's own tracer: they are inputs here, not results under test."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+SAMPLE = 4096
+
+
+def _run(hcc, name, bounce):
+    import hcc_inputs
+    import oracle
+    from hcc_inputs import rng as hrng
+    w = hcc_inputs.Workload(name)
+    b = w.bvh
+    bvh = hcc.Bvh(b.nodes, b.tris, b.prim_idx)
+
+    def gpu_trace(_b, rays):
+        t, p, _, _ = hcc.hits_to_numpy(hcc.trace(bvh, torch.from_numpy(rays).cuda(), None, hcc.TRACE_CLOSEST))
+        return t, p
+    diffuse, shadow = w.first_bounce(gpu_trace)
+    for b_i in range(2, bounce + 1):
+        t, p = gpu_trace(None, diffuse)
+        diffuse, shadow, _ = w.bounce(b_i, diffuse, t, p)
+    had = hcc.density(bvh)
+    assert np.array_equal(had.cpu().numpy().view(np.uint32), oracle.had(b.nodes).view(np.uint32))
+    cut = hcc.select_cut(bvh, had, w.K, w.key_bits)
+    tables, _, _ = oracle.select_cut(b.nodes, w.K, w.key_bits)
+    ent, cnt = cut.read()
+    assert np.array_equal(ent, tables.entry_node) and np.array_equal(cnt, tables.table_cnt)
+    info = cut.info()
+    pipe = hcc.Pipeline(shadow.shape[0], 64)
+    for rays_h, mode in ((diffuse, hcc.TRACE_CLOSEST), (shadow, hcc.TRACE_ANY)):
+        n = rays_h.shape[0]
+        rays = torch.from_numpy(rays_h).cuda()
+        perm = torch.empty(n, dtype=torch.int32, device="cuda")
+        hits = pipe.reorder_trace(bvh, cut, hcc.ORDER_HCC, rays, mode, perm_out=perm, key_bits=w.key_bits)
+        keys = hcc.encode(rays, cut)
+        # ---- permutation: the properties that define it
+        p64 = perm.to(torch.int64)
+        assert int(torch.bincount(p64, minlength=n).max()) == 1 and int(p64.min()) == 0 and int(p64.max()) == n - 1
+        ks = keys[p64]
+        if ks.dtype == torch.int32:
+            ks = ks.to(torch.int64) & 0xFFFFFFFF
+        dk = ks[1:] - ks[:-1]
+        assert info["bits_used"] < 64 and bool((dk >= 0).all())
+        tie = dk == 0
+        assert bool((p64[1:][tie] > p64[:-1][tie]).all())
+        # ---- sampled keys and hits against the oracle
+        idx = np.unique((hrng.u01(0x5A3B1E + n, 0, np.arange(SAMPLE, dtype=np.uint64), 0) * n).astype(np.int64))
+        sub = np.ascontiguousarray(rays_h[idx])
+        got_keys = hcc.keys_to_numpy(keys[torch.from_numpy(idx).cuda()]).astype(np.uint64)
+        assert np.array_equal(got_keys, oracle.encode_hcc(sub, b.nodes, tables))
+        if mode == hcc.TRACE_CLOSEST:
+            t, p, _, _ = hcc.hits_to_numpy(hits[torch.from_numpy(idx).cuda()])
+            wt, wp, _, _ = oracle.closest_bvh(sub, b.nodes, b.prim_idx, b.tris)
+            assert np.array_equal(np.isinf(t), np.isinf(wt))
+            h = ~np.isinf(wt)
+            assert np.all(np.abs(t[h] - wt[h]) <= 1e-5 * np.abs(wt[h]))
+            diff = np.nonzero(p != wp)[0]
+            for i in diff:      # a different prim id is right only when the two nearest t are within 1e-5 relative
+                ts = sorted(float(oracle.tri_hit(sub[i], tri)[1][0]) for tri in b.tris.reshape(-1, 9)[[p[i], wp[i]]])
+                assert ts[1] - ts[0] <= 1e-5 * abs(ts[0])
+            assert diff.shape[0] <= 8
+        else:
+            occ = hits[torch.from_numpy(idx).cuda()].cpu().numpy()
+            assert np.array_equal(occ, oracle.any_bvh(sub, b.nodes, b.prim_idx, b.tris))
+        del rays, perm, hits, keys
+    return diffuse.shape[0], shadow.shape[0]
+
+
+@pytest.fixture(scope="module")
+def hcc():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2305_16652_b200 as h
+    return h
+
+
+def test_config2_full_size(hcc):
+    n_d, n_s = _run(hcc, "room", 1)
+    assert n_d == 1048576 and n_s == 2097152
+
+
+def test_config3_full_size_second_bounce(hcc):
+    """Config 3 (~1 M triangles, 1920x1080x8 spp, 64-bit keys 16x16x16), the rays of bounce 2."""
+    n_d, n_s = _run(hcc, "fig1", 2)
+    assert n_d > 16_000_000 and n_s > 32_000_000
