@@ -470,9 +470,21 @@ def run_ours(args):
     hits_pin = {"diffuse": torch.empty((n_d, 4), dtype=torch.float32).pin_memory(),
                 "shadow": torch.empty(n_s, dtype=torch.uint8).pin_memory()}
 
+    # one pipeline and one stream per batch: the shadow batch's host->device copy overlaps the diffuse
+    # batch's kernels, the diffuse hits go back while the shadow batch is traced
+    pipes_h = {"diffuse": hcc.Pipeline(n_d, 64, host_staging=True), "shadow": pipe}
+    streams_h = {"diffuse": torch.cuda.Stream(), "shadow": torch.cuda.Stream()}
+
     def step_host():
+        cur = torch.cuda.current_stream()
         for _, mode, name in batches:
-            pipe.reorder_trace_host(bvh, cut, hcc.ORDER_HCC, rays_pin[name], hits_pin[name], mode, key_bits=w.key_bits)
+            st = streams_h[name]
+            st.wait_stream(cur)
+            pipes_h[name].reorder_trace_host_async(bvh, cut, hcc.ORDER_HCC, rays_pin[name], hits_pin[name], mode,
+                                                   key_bits=w.key_bits, stream=st)
+        for name in ("diffuse", "shadow"):
+            pipes_h[name].synchronize()
+            cur.wait_stream(streams_h[name])
     for _ in range(3):
         step_host()
     torch.cuda.synchronize()

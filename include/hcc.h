@@ -279,6 +279,15 @@ HCC_API int32_t hcc_reorder_trace(hcc_pipeline *p, const hcc_bvh *bvh, const hcc
 HCC_API int32_t hcc_reorder_trace_host(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
                                uint32_t key_bits, const float *rays_host, uint64_t n, int32_t mode,
                                void *hits_host, void *stream);
+/* The same without the final synchronisation: the call only enqueues on `stream` (the copies are
+ * asynchronous if the host buffers are pinned); hits_host is valid after hcc_pipeline_synchronize
+ * (or a synchronisation of `stream`).  Two pipelines on two streams overlap one batch's copies with
+ * the other batch's kernels. */
+HCC_API int32_t hcc_reorder_trace_host_async(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
+                                     uint32_t key_bits, const float *rays_host, uint64_t n, int32_t mode,
+                                     void *hits_host, void *stream);
+/* Waits until the pipeline's last enqueued call has finished. */
+HCC_API int32_t hcc_pipeline_synchronize(hcc_pipeline *p);
 /* Device time of the stages of the pipeline's last call, from CUDA events recorded on its
  * stream between the stages: ms[0] encode, [1] sort, [2] trace, [3] host->device copy,
  * [4] device->host copy (3, 4 = 0 for the device form).  Waits for that call to finish. */

@@ -52,6 +52,8 @@ _SIGNATURES = {
     "hcc_pipeline_destroy": [_vp],
     "hcc_reorder_trace": [_vp, _vp, _vp, _i32, _u32, _vp, _u64, _i32, _vp, _vp, _vp],
     "hcc_reorder_trace_host": [_vp, _vp, _vp, _i32, _u32, _vp, _u64, _i32, _vp, _vp],
+    "hcc_reorder_trace_host_async": [_vp, _vp, _vp, _i32, _u32, _vp, _u64, _i32, _vp, _vp],
+    "hcc_pipeline_synchronize": [_vp],
     "hcc_pipeline_stage_ms": [_vp, _vp],
     "hcc_trace_stats": [_vp, _vp, _u64, _vp, _i32, _vp, _vp, _vp],
     "hcc_anc": [_vp, _vp, _u64, _u32, _vp, _vp],
@@ -388,6 +390,20 @@ class Pipeline:
         _check(lib().hcc_reorder_trace_host(self._h, bvh._h, _vp(0) if cut is None else cut._h, int(order),
                                             int(key_bits), _vp(rp), n, int(mode), _vp(hp), _stream(stream)))
         return hits_host
+
+    def reorder_trace_host_async(self, bvh, cut, order, rays_host, hits_host, mode=TRACE_CLOSEST, key_bits=32,
+                                 stream=None):
+        """hcc_reorder_trace_host_async: enqueue only; hits_host is valid after synchronize()."""
+        n = rays_host.shape[0]
+        rp = rays_host.data_ptr() if isinstance(rays_host, torch.Tensor) else rays_host.ctypes.data
+        hp = hits_host.data_ptr() if isinstance(hits_host, torch.Tensor) else hits_host.ctypes.data
+        _check(lib().hcc_reorder_trace_host_async(self._h, bvh._h, _vp(0) if cut is None else cut._h, int(order),
+                                                  int(key_bits), _vp(rp), n, int(mode), _vp(hp), _stream(stream)))
+        return hits_host
+
+    def synchronize(self):
+        """hcc_pipeline_synchronize: wait for the pipeline's last enqueued call."""
+        _check(lib().hcc_pipeline_synchronize(self._h))
 
     def stage_ms(self):
         """dict(encode, sort, trace, h2d, d2h) in ms for the last call (waits for it)."""

@@ -137,9 +137,9 @@ extern "C" int32_t hcc_reorder_trace(hcc_pipeline *p, const hcc_bvh *bvh, const 
     return HCC_OK;
 }
 
-extern "C" int32_t hcc_reorder_trace_host(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
-                                          uint32_t key_bits, const float *rays_host, uint64_t n, int32_t mode,
-                                          void *hits_host, void *stream) {
+extern "C" int32_t hcc_reorder_trace_host_async(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
+                                                uint32_t key_bits, const float *rays_host, uint64_t n, int32_t mode,
+                                                void *hits_host, void *stream) {
     HCC_REQUIRE(p && p->host_staging, HCC_ERR_INVALID_ARG, "hcc_reorder_trace_host: pipeline created without host staging");
     HCC_REQUIRE(n <= p->n_max, HCC_ERR_INVALID_ARG, "hcc_reorder_trace_host: n exceeds the pipeline's n_max");
     HCC_REQUIRE(mode == HCC_TRACE_CLOSEST || mode == HCC_TRACE_ANY, HCC_ERR_INVALID_ARG, "hcc_reorder_trace_host: unknown mode %d", mode);
@@ -152,8 +152,23 @@ extern "C" int32_t hcc_reorder_trace_host(hcc_pipeline *p, const hcc_bvh *bvh, c
     if (rc != HCC_OK) return rc;
     HCC_CUDA_TRY(cudaMemcpyAsync(hits_host, p->d_hits, (mode == HCC_TRACE_CLOSEST ? 16 : 1) * n, cudaMemcpyDeviceToHost, s));
     HCC_CUDA_TRY(cudaEventRecord(p->ev[5], s));
-    HCC_CUDA_TRY(cudaStreamSynchronize(s));
     p->timed_host = true;
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_pipeline_synchronize(hcc_pipeline *p) {
+    HCC_REQUIRE(p, HCC_ERR_INVALID_ARG, "hcc_pipeline_synchronize: NULL pipeline");
+    if (!p->timed) return HCC_OK;
+    HCC_CUDA_TRY(cudaEventSynchronize(p->ev[p->timed_host ? 5 : 4]));
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_reorder_trace_host(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
+                                          uint32_t key_bits, const float *rays_host, uint64_t n, int32_t mode,
+                                          void *hits_host, void *stream) {
+    int32_t rc = hcc_reorder_trace_host_async(p, bvh, cut, order, key_bits, rays_host, n, mode, hits_host, stream);
+    if (rc != HCC_OK || n == 0) return rc;
+    HCC_CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
     return HCC_OK;
 }
 

@@ -133,3 +133,30 @@ def test_grid_pipeline_and_errors(hcc, cases):
     for bad, bits in (([3], 16), ([16, 16, 16], 32), ([1], 16)):
         with pytest.raises(hcc.HccError):
             hcc.select_grid(d["bvh"], bad, bits)
+
+
+# ------------------------------------------------------------------ host-buffer path, asynchronous form
+def test_reorder_trace_host_async_matches_the_device_path(hcc, cases):
+    """hcc_reorder_trace_host_async on two pipelines / two streams (bench.py's e2e leg) returns the
+    same bytes as the device-buffer call."""
+    d = cases["room_mid"]
+    cut = hcc.select_cut(d["bvh"], hcc.density(d["bvh"]), 1024, 32)
+    n_d, n_s = d["diffuse"].shape[0], d["shadow"].shape[0]
+    pa, pb = hcc.Pipeline(n_d, 64, host_staging=True), hcc.Pipeline(n_s, 64, host_staging=True)
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    rays_a = torch.from_numpy(d["case"].diffuse).pin_memory()
+    rays_b = torch.from_numpy(d["case"].shadow).pin_memory()
+    hits_a = torch.empty((n_d, 4), dtype=torch.float32).pin_memory()
+    hits_b = torch.empty(n_s, dtype=torch.uint8).pin_memory()
+    torch.cuda.synchronize()
+    for _ in range(3):
+        hits_a.zero_(); hits_b.zero_()
+        pa.reorder_trace_host_async(d["bvh"], cut, hcc.ORDER_HCC, rays_a, hits_a, hcc.TRACE_CLOSEST, stream=sa)
+        pb.reorder_trace_host_async(d["bvh"], cut, hcc.ORDER_HCC, rays_b, hits_b, hcc.TRACE_ANY, stream=sb)
+        pa.synchronize(); pb.synchronize()
+        ref_a = hcc.trace(d["bvh"], d["diffuse"], None, hcc.TRACE_CLOSEST)
+        ref_b = hcc.trace(d["bvh"], d["shadow"], None, hcc.TRACE_ANY)
+        assert torch.equal(hits_a.cuda().view(torch.int32), ref_a.view(torch.int32))
+        assert torch.equal(hits_b.cuda(), ref_b)
+    ms = pa.stage_ms()
+    assert ms["h2d"] > 0 and ms["trace"] > 0
