@@ -462,6 +462,19 @@ def run_ours(args):
             "hcc": run_order(hcc_keys(cut), info["bits_used"]),
             "grid": run_order(hcc_keys(grid_cut), info["bits_used"]),
             "ppc": run_order(lambda rays, keys=None: hcc.encode_ppc(bvh, rays, w.key_bits, keys=keys), w.key_bits)}
+        # config 4 of BASELINE.json: cut size x key length on the same rays (Tables 6-7 analogue)
+        sweep = []
+        for kb in (16, 24, 32, 48, 64):
+            tp = run_order(lambda rays, keys=None, kb=kb: hcc.encode_twopoint(rays, bvh.scene_lo, bvh.scene_hi, kb, keys=keys), 6 * (kb // 6))
+            sweep.append({"order": "twopoint", "key_bits": kb, "bits_used": 6 * (kb // 6), **tp})
+            for K in (256, 1024, 4096, 16384, 65536):
+                cut_s = hcc.select_cut(bvh, had, K, kb)
+                i_s = cut_s.info()
+                if any(e["order"] == "hcc" and e["key_bits"] == kb and e["widths"] == i_s["widths"] for e in sweep):
+                    continue      # capped to a hierarchy already measured at this key length
+                sweep.append({"order": "hcc", "key_bits": kb, "K": K, "K_eff": i_s["K_eff"], "widths": i_s["widths"],
+                              "bits_used": i_s["bits_used"], **run_order(hcc_keys(cut_s), i_s["bits_used"])})
+        studies["sweep"] = sweep
         studies["note"] = ("per batch medians of 5; grid = regular-grid tables of the same widths through the same encoder; "
                            "ppc = prefix path code with key_bits tests (upper-bound ordering, PAPER.md:128)")
 
