@@ -9,11 +9,26 @@ namespace hcc {
 constexpr int RADIX_BITS = 8;
 constexpr int RADIX = 1 << RADIX_BITS;
 // Tile shape per key width (4096 pairs per CTA either way): 256 threads x 16 pairs for 32-bit
-// keys, 512 x 8 for 64-bit keys; launch bounds cap the registers (4 resp. 3 CTAs per SM)
+// keys, 512 x 8 for 64-bit keys (overridable at build time for tuning); launch bounds cap the registers (4 resp. 3 CTAs per SM)
 // because occupancy, not bandwidth, decides this kernel's speed.
-template <typename KeyT> struct SortCfg { static constexpr int THREADS = 256, ITEMS = 16, MIN_CTAS = 4; };
-template <> struct SortCfg<unsigned long long> { static constexpr int THREADS = 512, ITEMS = 8, MIN_CTAS = 3; };
-constexpr int SORT_TILE = 4096;
+#ifndef HCC_SORT32_THREADS
+#define HCC_SORT32_THREADS 256
+#define HCC_SORT32_ITEMS 16
+#define HCC_SORT32_MIN_CTAS 4
+#endif
+#ifndef HCC_SORT64_THREADS
+#define HCC_SORT64_THREADS 512
+#define HCC_SORT64_ITEMS 8
+#define HCC_SORT64_MIN_CTAS 3
+#endif
+template <typename KeyT> struct SortCfg {
+    static constexpr int THREADS = HCC_SORT32_THREADS, ITEMS = HCC_SORT32_ITEMS, MIN_CTAS = HCC_SORT32_MIN_CTAS;
+};
+template <> struct SortCfg<unsigned long long> {
+    static constexpr int THREADS = HCC_SORT64_THREADS, ITEMS = HCC_SORT64_ITEMS, MIN_CTAS = HCC_SORT64_MIN_CTAS;
+};
+constexpr int SORT_TILE = HCC_SORT32_THREADS * HCC_SORT32_ITEMS;
+static_assert(HCC_SORT64_THREADS * HCC_SORT64_ITEMS == SORT_TILE, "both key widths use the same tile size");
 constexpr int MAX_PASSES = 8;
 constexpr uint32_t FLAG_AGG = 1u << 30, FLAG_PREFIX = 2u << 30, VAL_MASK = (1u << 30) - 1u;
 constexpr int HIST_THREADS = 256;
