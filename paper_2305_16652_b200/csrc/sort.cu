@@ -32,14 +32,18 @@ static_assert(HCC_SORT64_THREADS * HCC_SORT64_ITEMS == SORT_TILE, "both key widt
 constexpr int MAX_PASSES = 8;
 constexpr uint32_t FLAG_AGG = 1u << 30, FLAG_PREFIX = 2u << 30, VAL_MASK = (1u << 30) - 1u;
 constexpr int HIST_THREADS = 256;
-constexpr uint32_t FEW_DIGITS = 16;
+constexpr int HIST_BATCH = 4;
+#ifndef HCC_SORT_FEW
+#define HCC_SORT_FEW 20
+#endif
+constexpr float MATCH_MAX_DISTINCT = (float)HCC_SORT_FEW;   // expected distinct digits per warp up to which MATCH.ANY is used
 constexpr int LOOK = 4;                      // look-back rows fetched per round trip
 
 // control region of the workspace (zeroed once per sort by one memset)
 struct SortCtl {
     uint32_t hist[MAX_PASSES][RADIX];
     uint32_t ticket[MAX_PASSES];
-    uint32_t few_digits[MAX_PASSES];   // pass p sees at most FEW_DIGITS distinct digit values
+    uint32_t few_digits[MAX_PASSES];   // pass p: a warp's 32 keys are expected to hold few distinct digits
 
 };
 
@@ -59,11 +63,31 @@ k_histogram(const KeyT *__restrict__ keys, uint32_t n, uint32_t passes, uint32_t
     __shared__ uint32_t sh[MAX_PASSES][RADIX];
     for (uint32_t i = threadIdx.x; i < MAX_PASSES * RADIX; i += HIST_THREADS) (&sh[0][0])[i] = 0u;
     __syncthreads();
+    // 16 bytes of keys per load and HIST_BATCH independent loads in flight per thread: the kernel is
+    // a pure stream and would otherwise wait one DRAM round trip per key
+    constexpr uint32_t PER = 16 / sizeof(KeyT);
+    const uint32_t n_vec = n / PER;
+    const uint4 *vec = reinterpret_cast<const uint4 *>(keys);
     const uint32_t stride = gridDim.x * HIST_THREADS;
-    for (uint32_t i = blockIdx.x * HIST_THREADS + threadIdx.x; i < n; i += stride) {
-        KeyT k = keys[i];
+    auto count = [&](KeyT k) {
         for (uint32_t p = 0; p < passes; ++p) atomicAdd(&sh[p][(uint32_t)(k >> (bit_lo + RADIX_BITS * p)) & (RADIX - 1)], 1u);
+    };
+    for (uint32_t i = blockIdx.x * HIST_THREADS + threadIdx.x; i < n_vec; i += HIST_BATCH * stride) {
+        uint4 v[HIST_BATCH];
+#pragma unroll
+        for (int b = 0; b < HIST_BATCH; ++b) {
+            const uint32_t j = i + b * stride;
+            v[b] = j < n_vec ? vec[j] : make_uint4(0u, 0u, 0u, 0u);
+        }
+#pragma unroll
+        for (int b = 0; b < HIST_BATCH; ++b) {
+            if (i + b * stride < n_vec) {
+                if (sizeof(KeyT) == 4) { count((KeyT)v[b].x); count((KeyT)v[b].y); count((KeyT)v[b].z); count((KeyT)v[b].w); }
+                else { count((KeyT)(((unsigned long long)v[b].y << 32) | v[b].x)); count((KeyT)(((unsigned long long)v[b].w << 32) | v[b].z)); }
+            }
+        }
     }
+    for (uint32_t i = n_vec * PER + blockIdx.x * HIST_THREADS + threadIdx.x; i < n; i += stride) count(keys[i]);   // ragged tail
     __syncthreads();
     for (uint32_t i = threadIdx.x; i < passes * RADIX; i += HIST_THREADS) {
         uint32_t c = (&sh[0][0])[i];
@@ -74,8 +98,9 @@ k_histogram(const KeyT *__restrict__ keys, uint32_t n, uint32_t passes, uint32_t
 // Exclusive scan of each digit histogram, written as the PREFIX row of "tile -1"
 // (row 0 of that pass's status array), so the look-back needs no special first tile.
 __global__ void __launch_bounds__(RADIX)
-k_scan_hist(SortCtl *ctl, uint32_t *status, size_t status_stride) {
+k_scan_hist(SortCtl *ctl, uint32_t *status, size_t status_stride, uint32_t n) {
     __shared__ uint32_t s_w[RADIX / 32];
+    __shared__ float s_e[RADIX / 32];
     const uint32_t p = blockIdx.x, d = threadIdx.x, lane = d & 31u, warp = d >> 5;
     uint32_t v = ctl->hist[p][d], incl = v;
 #pragma unroll
@@ -84,8 +109,18 @@ k_scan_hist(SortCtl *ctl, uint32_t *status, size_t status_stride) {
         if (lane >= (uint32_t)o) incl += x;
     }
     if (lane == 31) s_w[warp] = incl;
-    const int distinct = __syncthreads_count(v != 0u);
-    if (d == 0) ctl->few_digits[p] = (uint32_t)distinct <= FEW_DIGITS ? 1u : 0u;
+    // expected number of distinct digits among the 32 keys of a warp = sum_d 1 - (1 - p_d)^32:
+    // MATCH.ANY costs a round per distinct value, the ballot form a fixed 9 rounds
+    float e = v ? 1.0f - exp2f(32.0f * log2f(fmaxf(1.0f - (float)v / (float)n, 1e-30f))) : 0.0f;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xFFFFFFFFu, e, o);
+    if (lane == 0) s_e[warp] = e;
+    __syncthreads();
+    if (d == 0) {
+        float tot = 0.0f;
+        for (int w = 0; w < RADIX / 32; ++w) tot += s_e[w];
+        ctl->few_digits[p] = tot <= MATCH_MAX_DISTINCT ? 1u : 0u;
+    }
     uint32_t add = 0;
     for (uint32_t w = 0; w < warp; ++w) add += s_w[w];
     status[p * status_stride + d] = FLAG_PREFIX | (add + incl - v);
@@ -256,10 +291,10 @@ static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t bit_l
     const size_t status_stride = (size_t)(tiles + 1) * RADIX;
     HCC_CUDA_TRY(cudaMemsetAsync(ctl_raw, 0, round_up(sizeof(SortCtl), 256) + (size_t)passes * status_stride * sizeof(uint32_t), s));
     int hist_blocks = (int)((n + HIST_THREADS * 16 - 1) / (HIST_THREADS * 16));
-    int cap = sm_count() * 4;
+    int cap = sm_count() * 8;
     if (hist_blocks > cap) hist_blocks = cap;
     k_histogram<KeyT><<<hist_blocks, HIST_THREADS, 0, s>>>(keys, n, passes, bit_lo, ctl);
-    k_scan_hist<<<passes, RADIX, 0, s>>>(ctl, status, status_stride);
+    k_scan_hist<<<passes, RADIX, 0, s>>>(ctl, status, status_stride, n);
     const size_t dyn = (sizeof(KeyT) + sizeof(uint32_t)) * SORT_TILE;
     constexpr int SORT_THREADS = SortCfg<KeyT>::THREADS;
     static bool attr_done = false;
