@@ -139,35 +139,43 @@ template <typename KeyT, bool FIRST, bool WRITE_KEYS>
 __global__ void __launch_bounds__(SortCfg<KeyT>::THREADS, SortCfg<KeyT>::MIN_CTAS)
 k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const uint32_t *__restrict__ vals_in,
            uint32_t *__restrict__ vals_out, uint32_t n, uint32_t shift, uint32_t *status, uint32_t *ticket,
-           const uint32_t *few_digits) {
+           const uint32_t *few_digits, uint32_t tiles) {
     constexpr int SORT_THREADS = SortCfg<KeyT>::THREADS, SORT_ITEMS = SortCfg<KeyT>::ITEMS, SORT_WARPS = SORT_THREADS / 32;
     static_assert(SORT_THREADS * SORT_ITEMS == SORT_TILE && SORT_THREADS >= RADIX, "tile shape");
     __shared__ uint32_t s_warp_hist[SORT_WARPS][RADIX];
     __shared__ uint32_t s_tile_off[RADIX];
     __shared__ uint32_t s_gbase[RADIX];
     __shared__ uint32_t s_warp_tot[RADIX / 32];
-    __shared__ uint32_t s_tile;
+    __shared__ uint32_t s_ticket[2];
     extern __shared__ __align__(16) unsigned char s_dyn[];
     KeyT *s_keys = reinterpret_cast<KeyT *>(s_dyn);
     uint32_t *s_vals = reinterpret_cast<uint32_t *>(s_dyn + sizeof(KeyT) * SORT_TILE);
 
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
-    for (uint32_t i = tid; i < SORT_WARPS * RADIX; i += SORT_THREADS) (&s_warp_hist[0][0])[i] = 0u;
-    __syncthreads();
-    const uint32_t tile = s_tile;
     const bool use_match = *few_digits != 0u;      // uniform over the grid
-    const uint32_t tile_base = tile * SORT_TILE;
-    const uint32_t count = min((uint32_t)SORT_TILE, n - tile_base);
     const uint32_t my_base = warp * (SORT_ITEMS * 32) + lane;   // item i at my_base + 32*i (warp-striped)
-
     KeyT key[SORT_ITEMS];
     uint32_t rank[SORT_ITEMS];
+    auto load_keys = [&](uint32_t t) {
+        const uint32_t base = t * SORT_TILE, cnt = min((uint32_t)SORT_TILE, n - base);
 #pragma unroll
-    for (int i = 0; i < SORT_ITEMS; ++i) {
-        uint32_t idx = my_base + 32 * i;
-        key[i] = idx < count ? keys_in[tile_base + idx] : (KeyT)0;
-    }
+        for (int i = 0; i < SORT_ITEMS; ++i) {
+            const uint32_t idx = my_base + 32 * i;
+            key[i] = idx < cnt ? keys_in[base + idx] : (KeyT)0;
+        }
+    };
+    if (tid == 0) s_ticket[0] = atomicAdd(ticket, 1u);
+    __syncthreads();
+    uint32_t tile = s_ticket[0], slot = 0;
+    if (tile < tiles) load_keys(tile);
+  while (tile < tiles) {                           // persistent: one CTA works through many tiles
+    for (uint32_t i = tid; i < SORT_WARPS * RADIX; i += SORT_THREADS) (&s_warp_hist[0][0])[i] = 0u;
+    if (tid == 0) s_ticket[slot ^ 1u] = atomicAdd(ticket, 1u);
+    __syncthreads();
+    const uint32_t next = s_ticket[slot ^ 1u];
+    const uint32_t tile_base = tile * SORT_TILE;
+    const uint32_t count = min((uint32_t)SORT_TILE, n - tile_base);
+
     // rank every item among the equal digits of its warp, in (item, lane) order
     const uint32_t lt = (1u << lane) - 1u;
 #pragma unroll
@@ -242,6 +250,10 @@ k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const 
         }
     }
 
+    // the key registers are free now: bring in the next tile's keys while this tile looks back and
+    // writes out
+    if (next < tiles) load_keys(next);
+
     // decoupled look-back over rows tile, tile-1, ..., 0 (row 0 = seeded global digit base).
     // LOOK rows are read at once: a walk over aggregates costs one L2 round trip per LOOK rows
     // instead of one per row.  Rows before row 0 are never reached logically (row 0 is a
@@ -273,6 +285,10 @@ k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const 
         if (WRITE_KEYS) keys_out[pos] = k;
         vals_out[pos] = s_vals[p];
     }
+    __syncthreads();                               // shared buffers and the ticket slot are reused by the next tile
+    tile = next;
+    slot ^= 1u;
+  }
 }
 
 static uint64_t ctl_bytes(uint64_t n) {
@@ -305,6 +321,10 @@ static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t bit_l
         HCC_CUDA_TRY(cudaFuncSetAttribute(k_onesweep<KeyT, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
         attr_done = true;
     }
+    int per_sm = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_onesweep<KeyT, false, true>, SORT_THREADS, dyn) != cudaSuccess || per_sm < 1) per_sm = 1;
+    const uint32_t resident = (uint32_t)(sm_count() * per_sm);
+    const uint32_t grid = tiles < resident ? tiles : resident;     // every CTA resident: the look-back cannot starve
     KeyT *kin = keys, *kout = keys_tmp;
     for (uint32_t p = 0; p < passes; ++p) {
         const bool first = p == 0, last = p + 1 == passes;
@@ -315,10 +335,10 @@ static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t bit_l
         uint32_t *tk = &ctl->ticket[p];
         const uint32_t *fd = &ctl->few_digits[p];
         const uint32_t shift = bit_lo + RADIX_BITS * p;
-        if (first && last) k_onesweep<KeyT, true, false><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd);
-        else if (first)    k_onesweep<KeyT, true, true><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd);
-        else if (last)     k_onesweep<KeyT, false, false><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd);
-        else               k_onesweep<KeyT, false, true><<<tiles, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd);
+        if (first && last) k_onesweep<KeyT, true, false><<<grid, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd, tiles);
+        else if (first)    k_onesweep<KeyT, true, true><<<grid, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd, tiles);
+        else if (last)     k_onesweep<KeyT, false, false><<<grid, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd, tiles);
+        else               k_onesweep<KeyT, false, true><<<grid, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd, tiles);
         KeyT *t = kin; kin = kout; kout = t;
     }
     HCC_CUDA_TRY(cudaGetLastError());
