@@ -8,17 +8,17 @@ namespace hcc {
 
 constexpr int RADIX_BITS = 8;
 constexpr int RADIX = 1 << RADIX_BITS;
-// Tile shape per key width (4096 pairs per CTA either way): 256 threads x 16 pairs for 32-bit
-// keys, 512 x 8 for 64-bit keys (overridable at build time for tuning); launch bounds cap the registers (4 resp. 3 CTAs per SM)
-// because occupancy, not bandwidth, decides this kernel's speed.
+// Tile shape (4096 pairs per CTA): 256 threads x 16 pairs for both key widths (overridable at build
+// time for tuning); launch bounds cap the registers at 4 (32-bit keys) resp. 3 (64-bit keys) CTAs
+// per SM because occupancy, not bandwidth, decides this kernel's speed.
 #ifndef HCC_SORT32_THREADS
 #define HCC_SORT32_THREADS 256
 #define HCC_SORT32_ITEMS 16
 #define HCC_SORT32_MIN_CTAS 4
 #endif
 #ifndef HCC_SORT64_THREADS
-#define HCC_SORT64_THREADS 512
-#define HCC_SORT64_ITEMS 8
+#define HCC_SORT64_THREADS 256
+#define HCC_SORT64_ITEMS 16
 #define HCC_SORT64_MIN_CTAS 3
 #endif
 template <typename KeyT> struct SortCfg {
@@ -32,7 +32,10 @@ static_assert(HCC_SORT64_THREADS * HCC_SORT64_ITEMS == SORT_TILE, "both key widt
 constexpr int MAX_PASSES = 8;
 constexpr uint32_t FLAG_AGG = 1u << 30, FLAG_PREFIX = 2u << 30, VAL_MASK = (1u << 30) - 1u;
 constexpr int HIST_THREADS = 256;
-constexpr int HIST_BATCH = 4;
+#ifndef HCC_HIST_BATCH
+#define HCC_HIST_BATCH 4
+#endif
+constexpr int HIST_BATCH = HCC_HIST_BATCH;
 #ifndef HCC_SORT_FEW
 #define HCC_SORT_FEW 20
 #endif
@@ -164,10 +167,24 @@ k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const 
             key[i] = idx < cnt ? keys_in[base + idx] : (KeyT)0;
         }
     };
+    // 64-bit keys also bring the next tile's ray ids in early (the 32-bit kernel has no registers to spare)
+    constexpr bool PREFETCH_VALS = !FIRST && sizeof(KeyT) == 8;
+    uint32_t val[PREFETCH_VALS ? SORT_ITEMS : 1];
+    auto load_vals = [&](uint32_t t) {
+        const uint32_t base = t * SORT_TILE, cnt = min((uint32_t)SORT_TILE, n - base);
+#pragma unroll
+        for (int i = 0; i < SORT_ITEMS; ++i) {
+            const uint32_t idx = my_base + 32 * i;
+            val[PREFETCH_VALS ? i : 0] = idx < cnt ? vals_in[base + idx] : 0u;
+        }
+    };
     if (tid == 0) s_ticket[0] = atomicAdd(ticket, 1u);
     __syncthreads();
     uint32_t tile = s_ticket[0], slot = 0;
-    if (tile < tiles) load_keys(tile);
+    if (tile < tiles) {
+        load_keys(tile);
+        if (PREFETCH_VALS) load_vals(tile);
+    }
   while (tile < tiles) {                           // persistent: one CTA works through many tiles
     for (uint32_t i = tid; i < SORT_WARPS * RADIX; i += SORT_THREADS) (&s_warp_hist[0][0])[i] = 0u;
     if (tid == 0) s_ticket[slot ^ 1u] = atomicAdd(ticket, 1u);
@@ -246,13 +263,16 @@ k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const 
             const uint32_t digit = (uint32_t)(key[i] >> shift) & (RADIX - 1);
             const uint32_t p = s_tile_off[digit] + s_warp_hist[warp][digit] + rank[i];
             s_keys[p] = key[i];
-            s_vals[p] = FIRST ? tile_base + idx : vals_in[tile_base + idx];
+            s_vals[p] = FIRST ? tile_base + idx : (PREFETCH_VALS ? val[PREFETCH_VALS ? i : 0] : vals_in[tile_base + idx]);
         }
     }
 
     // the key registers are free now: bring in the next tile's keys while this tile looks back and
     // writes out
-    if (next < tiles) load_keys(next);
+    if (next < tiles) {
+        load_keys(next);
+        if (PREFETCH_VALS) load_vals(next);
+    }
 
     // decoupled look-back over rows tile, tile-1, ..., 0 (row 0 = seeded global digit base).
     // LOOK rows are read at once: a walk over aggregates costs one L2 round trip per LOOK rows
