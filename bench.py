@@ -44,7 +44,7 @@ UNIT = "Mrays/s"
 OPS_BOX, OPS_PAIR, OPS_TRI = 26, 34, 36
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the two trace kernels on config 2, from the
 # ncu --set full capture summarised in profiles/r1b_ncu_full.md (a profiler number, config "room" only)
-NCU_TRAFFIC_ROOM = {"diffuse": 41.134336e6 + 0.591872e6, "shadow": 79.224832e6 + 3.907840e6}
+NCU_TRAFFIC_ROOM = {"diffuse": 41.140480e6 + 0.928000e6, "shadow": 79.290880e6 + 5.325568e6}
 SM_COUNT, LANES_PER_SM = 148, 128
 
 
