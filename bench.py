@@ -462,6 +462,9 @@ def run_ours(args):
             "hcc": run_order(hcc_keys(cut), info["bits_used"]),
             "grid": run_order(hcc_keys(grid_cut), info["bits_used"]),
             "ppc": run_order(lambda rays, keys=None: hcc.encode_ppc(bvh, rays, w.key_bits, keys=keys), w.key_bits)}
+        if len(info["widths"]) > 1:      # Algorithm 3 as printed (small popped nodes dropped) instead of reading R4
+            lit_cut = hcc.select_cut_levels(bvh, had, info["widths"], w.key_bits, flags=hcc.CUT_ALG3_DISCARD)
+            studies["orders"]["hcc_alg3_discard"] = run_order(hcc_keys(lit_cut), info["bits_used"])
         # config 4 of BASELINE.json: cut size x key length on the same rays (Tables 6-7 analogue)
         sweep = []
         for kb in (16, 24, 32, 48, 64):

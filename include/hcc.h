@@ -141,6 +141,16 @@ HCC_API int32_t hcc_select_cut(const hcc_bvh *bvh, const float *density_dev, uin
 /* Same with explicit level widths (each 1..64, m <= HCC_MAX_LEVELS, sum <= key_bits). */
 HCC_API int32_t hcc_select_cut_levels(const hcc_bvh *bvh, const float *density_dev, const uint32_t *widths_host,
                               uint32_t m, uint32_t key_bits, hcc_cut *cut, void *stream);
+
+/* (f4) The same with flags.  HCC_CUT_ALG3_DISCARD: every level that has a level below it is built by
+ * Algorithm 3 as printed ("we discard the top-level node that does not have a
+ * sufficient subtree ... This ensures that there are no empty low-level nodes"): a popped node with fewer
+ * leaves below it than the next level's width is dropped instead of being kept as an entry.  Tables may
+ * then hold fewer entries, leave parts of the scene covered by no entry, or be empty; the last level is
+ * Algorithm 2 either way.  flags = 0 is hcc_select_cut_levels. */
+#define HCC_CUT_ALG3_DISCARD 1u
+HCC_API int32_t hcc_select_cut_levels_ex(const hcc_bvh *bvh, const float *density_dev, const uint32_t *widths,
+                                 uint32_t m, uint32_t key_bits, uint32_t flags, hcc_cut *cut, void *stream);
 /* Shape of the last selection (host values, no synchronisation): number of levels, their
  * widths (array of HCC_MAX_LEVELS), K actually used, key bits used = sum of widths, key
  * container bits (32 or 64), total entries and tables over all levels. Out pointers may be NULL. */

@@ -33,6 +33,10 @@ def _load():
         L.oracle_cut.restype = _u32
         L.oracle_level_tables.argtypes = [_vp, _vp, _vp, _vp, _u32, _vp, _vp]
         L.oracle_level_tables.restype = None
+        L.oracle_level_tables_ex.argtypes = [_vp, _vp, _vp, _vp, _u32, ctypes.c_int, _vp, _vp]
+        L.oracle_level_tables_ex.restype = None
+        L.oracle_cut_ex.argtypes = [_vp, _vp, _vp, _u32, _u32, _u32, ctypes.c_int, _vp]
+        L.oracle_cut_ex.restype = _u32
         L.oracle_slab_hit.argtypes = [_vp, _vp, _vp]
         L.oracle_slab_hit.restype = ctypes.c_int
         L.oracle_encode_hcc.argtypes = [_vp, _u64, _vp, _vp, _u32, _vp, _vp, _vp]
@@ -90,17 +94,18 @@ def subtree_leaves(nodes):
     return out
 
 
-def cut(nodes, had_, K, start=0, need=2, leaves=None):
+def cut(nodes, had_, K, start=0, need=2, leaves=None, discard=False):
     """Cut(start, K, need): Algorithm 2 from `start`; need > 2 gives
-    Algorithm 3's "large enough subtree" test.  Node ids, HAD-descending."""
+    Algorithm 3's "large enough subtree" test; discard=True is the literal Algorithm 3 (a node
+    that is not large enough is dropped).  Node ids, HAD-descending (:192)."""
     nodes = _c(nodes)
     had_ = _c(had_, np.float32)
     if leaves is None:
         leaves = subtree_leaves(nodes)
     leaves = _c(leaves, np.uint32)
     out = np.empty(max(int(K), 1), dtype=np.uint32)
-    n = _load().oracle_cut(nodes.ctypes.data, had_.ctypes.data, leaves.ctypes.data,
-                           int(start), int(K), int(need), out.ctypes.data)
+    n = _load().oracle_cut_ex(nodes.ctypes.data, had_.ctypes.data, leaves.ctypes.data,
+                              int(start), int(K), int(need), 1 if discard else 0, out.ctypes.data)
     return out[:n].copy()
 
 
@@ -159,7 +164,7 @@ class Tables:
         return e[e != INVALID]
 
 
-def level_tables(nodes, had_, widths, leaves=None):
+def level_tables(nodes, had_, widths, leaves=None, discard=False):
     nodes = _c(nodes)
     had_ = _c(had_, np.float32)
     if leaves is None:
@@ -172,8 +177,9 @@ def level_tables(nodes, had_, widths, leaves=None):
         n_ent += nt * int(x); n_tab += nt; nt *= int(x)
     entry_node = np.empty(n_ent, dtype=np.uint32)
     table_cnt = np.empty(n_tab, dtype=np.uint32)
-    _load().oracle_level_tables(nodes.ctypes.data, had_.ctypes.data, leaves.ctypes.data,
-                                w.ctypes.data, len(w), entry_node.ctypes.data, table_cnt.ctypes.data)
+    _load().oracle_level_tables_ex(nodes.ctypes.data, had_.ctypes.data, leaves.ctypes.data,
+                                   w.ctypes.data, len(w), 1 if discard else 0, entry_node.ctypes.data,
+                                   table_cnt.ctypes.data)
     return Tables(w, entry_node, table_cnt)
 
 

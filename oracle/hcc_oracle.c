@@ -127,9 +127,13 @@ static int cmp_cut(const void *a, const void *b) {
  *   R5: line 10 "Push the child" = push both children.  R6: the loop also stops when the
  *   queue is empty (a BVH with fewer than max_size leaves), so the result is all leaves.
  *   Output: sorted by HAD descending, ties -> lower index.
- * Returns the number of cut nodes written to out (<= max_size). */
-uint32_t oracle_cut(const node_t *nodes, const float *had, const uint32_t *leaves,
-                    uint32_t start, uint32_t max_size, uint32_t need, uint32_t *out) {
+ * Returns the number of cut nodes written to out (<= max_size).
+ * discard != 0 (f4, the literal Algorithm 3, "we discard the top-level
+ *   node that does not have a sufficient subtree"): a popped node that is not expandable is
+ *   dropped - not added to the list, MaxQueueSize unchanged (Alg. 3 has no lines 7-8).  The
+ *   result may then leave leaves uncovered and may be empty. */
+uint32_t oracle_cut_ex(const node_t *nodes, const float *had, const uint32_t *leaves,
+                       uint32_t start, uint32_t max_size, uint32_t need, int discard, uint32_t *out) {
     if (max_size == 0) return 0;
     heap_t pq;
     pq.v = (uint32_t *)malloc(sizeof(uint32_t) * ((size_t)max_size + 2));
@@ -141,8 +145,10 @@ uint32_t oracle_cut(const node_t *nodes, const float *had, const uint32_t *leave
         uint32_t nd = heap_pop(&pq, had);     /* line 5 */
         int expandable = nodes[nd].count == 0 && leaves[nd] >= need;
         if (!expandable) {                    /* line 6 */
-            out[n_out++] = nd;                /* line 7 */
-            max_queue -= 1;                   /* line 8 */
+            if (!discard) {
+                out[n_out++] = nd;            /* line 7 */
+                max_queue -= 1;               /* line 8 */
+            }                                 /* Alg. 3: the node is simply gone */
         } else {                              /* line 9 */
             heap_push(&pq, had, nodes[nd].left_or_first);      /* line 10 */
             heap_push(&pq, had, nodes[nd].left_or_first + 1);
@@ -155,6 +161,11 @@ uint32_t oracle_cut(const node_t *nodes, const float *had, const uint32_t *leave
     return n_out;
 }
 
+uint32_t oracle_cut(const node_t *nodes, const float *had, const uint32_t *leaves,
+                    uint32_t start, uint32_t max_size, uint32_t need, uint32_t *out) {
+    return oracle_cut_ex(nodes, had, leaves, start, max_size, need, 0, out);
+}
+
 /* Multi-level tables (MLHCC, generalised to m levels by reading
  * R-ML of SURVEY.md §8(c)-A / DESIGN.md):
  *   level 0 has one table  = Cut(root, w[0], need_0)
@@ -162,9 +173,12 @@ uint32_t oracle_cut(const node_t *nodes, const float *had, const uint32_t *leave
  *                          = Cut(node(e), w[l], need_l);  an empty entry has an empty table
  *   need_l = w[l+1] for l < m-1, and 2 on the last level (pure Alg. 2).
  * entry_node: concatenation over levels of n_tables[l]*w[l] node ids (INVALID_U32 = empty);
- * table_cnt:  concatenation over levels of n_tables[l] entry counts. */
-void oracle_level_tables(const node_t *nodes, const float *had, const uint32_t *leaves,
-                         const uint32_t *w, uint32_t m, uint32_t *entry_node, uint32_t *table_cnt) {
+ * table_cnt:  concatenation over levels of n_tables[l] entry counts.
+ * discard != 0: every level that has a level below it is built by the literal Algorithm 3
+ * (oracle_cut_ex with discard); the last level is Algorithm 2 either way ("follows a
+ * similar method as HCC"). */
+void oracle_level_tables_ex(const node_t *nodes, const float *had, const uint32_t *leaves,
+                            const uint32_t *w, uint32_t m, int discard, uint32_t *entry_node, uint32_t *table_cnt) {
     size_t ent_off = 0, tab_off = 0, prev_ent_off = 0;
     size_t n_tables = 1;
     for (uint32_t l = 0; l < m; ++l) {
@@ -174,7 +188,7 @@ void oracle_level_tables(const node_t *nodes, const float *had, const uint32_t *
             for (uint32_t j = 0; j < w[l]; ++j) dst[j] = INVALID_U32;
             uint32_t start = (l == 0) ? 0u : entry_node[prev_ent_off + t];
             uint32_t c = 0;
-            if (start != INVALID_U32) c = oracle_cut(nodes, had, leaves, start, w[l], need, dst);
+            if (start != INVALID_U32) c = oracle_cut_ex(nodes, had, leaves, start, w[l], need, discard && l + 1 < m, dst);
             table_cnt[tab_off + t] = c;
         }
         prev_ent_off = ent_off;
@@ -182,6 +196,11 @@ void oracle_level_tables(const node_t *nodes, const float *had, const uint32_t *
         tab_off += n_tables;
         n_tables *= w[l];
     }
+}
+
+void oracle_level_tables(const node_t *nodes, const float *had, const uint32_t *leaves,
+                         const uint32_t *w, uint32_t m, uint32_t *entry_node, uint32_t *table_cnt) {
+    oracle_level_tables_ex(nodes, had, leaves, w, m, 0, entry_node, table_cnt);
 }
 
 /* ------------------------------------------------------------------------- */

@@ -34,6 +34,7 @@ _SIGNATURES = {
     "hcc_cut_destroy": [_vp],
     "hcc_select_cut": [_vp, _vp, _u32, _u32, _vp, _vp],
     "hcc_select_cut_levels": [_vp, _vp, _vp, _u32, _u32, _vp, _vp],
+    "hcc_select_cut_levels_ex": [_vp, _vp, _vp, _u32, _u32, _u32, _vp, _vp],
     "hcc_cut_info": [_vp, _pu32, _pu32, _pu32, _pu32, _pu32, _pu64, _pu64],
     "hcc_cut_read": [_vp, _vp, _vp, _vp],
     "hcc_select_cut_flat_workspace_bytes": [_vp, _u32, _pu64],
@@ -205,12 +206,17 @@ def select_cut(bvh, density_dev, K, key_bits, cut=None, stream=None):
     return cut
 
 
-def select_cut_levels(bvh, density_dev, widths, key_bits, cut=None, stream=None):
+CUT_ALG3_DISCARD = 1
+
+
+def select_cut_levels(bvh, density_dev, widths, key_bits, cut=None, stream=None, flags=0):
+    """hcc_select_cut_levels(_ex): level tables of explicit widths; flags=CUT_ALG3_DISCARD builds the upper
+    levels by Algorithm 3 as printed."""
     w = np.ascontiguousarray(widths, dtype=np.uint32)
     if cut is None:
         cut = Cut(max(int(np.prod(w.astype(np.int64))), 64))
-    _check(lib().hcc_select_cut_levels(bvh._h, _dev(density_dev, (torch.float32,), "density"), w.ctypes.data,
-                                       w.shape[0], int(key_bits), cut._h, _stream(stream)))
+    _check(lib().hcc_select_cut_levels_ex(bvh._h, _dev(density_dev, (torch.float32,), "density"), w.ctypes.data,
+                                          w.shape[0], int(key_bits), int(flags), cut._h, _stream(stream)))
     return cut
 
 

@@ -89,6 +89,7 @@ struct hcc_bvh {
 struct hcc_cut {
     uint32_t cap_entries, cap_tables;
     uint32_t K_eff, key_bits, container_bits;
+    uint32_t flags;         // HCC_CUT_* of the last selection
     hcc::CutDev dev;        // pointers into the buffers below
     float4 *d_boxes;
     uint32_t *d_entry_node;

@@ -40,7 +40,7 @@ constexpr int TABLE_WARPS = 4;
 __global__ void __launch_bounds__(TABLE_WARPS * 32)
 k_build_tables(const hcc_node *__restrict__ nodes, const float *__restrict__ had,
                const uint32_t *__restrict__ leaves, const uint32_t *__restrict__ parent_entries,
-               uint32_t n_tables, uint32_t w, uint32_t need, uint32_t *__restrict__ entry_node,
+               uint32_t n_tables, uint32_t w, uint32_t need, uint32_t discard, uint32_t *__restrict__ entry_node,
                uint32_t *__restrict__ table_cnt, float4 *__restrict__ boxes) {
     __shared__ unsigned long long s_q[TABLE_WARPS][64];
     __shared__ unsigned long long s_out[TABLE_WARPS][64];
@@ -71,8 +71,13 @@ k_build_tables(const hcc_node *__restrict__ nodes, const float *__restrict__ had
             uint32_t count = nodes[node].count, left = nodes[node].left_or_first;
             bool expandable = count == 0 && leaves[node] >= need;
             if (!expandable) {
-                if (lane == 0) { out[n_out] = gmax; q[gslot] = 0ull; }
-                ++n_out; --maxq; --len;
+                if (discard) {              // literal Algorithm 3: the node is dropped
+                    if (lane == 0) q[gslot] = 0ull;
+                    --len;
+                } else {                    // Algorithm 2 lines 6-8: retired into the list
+                    if (lane == 0) { out[n_out] = gmax; q[gslot] = 0ull; }
+                    ++n_out; --maxq; --len;
+                }
             } else {
                 if (lane == 0) q[gslot] = make_key(had, left);
                 __syncwarp();
@@ -121,6 +126,7 @@ int32_t launch_build_tables(const hcc_bvh *bvh, const float *had, hcc_cut *cut, 
         uint32_t blocks = (d.n_tab[l] + TABLE_WARPS - 1) / TABLE_WARPS;
         k_build_tables<<<blocks, TABLE_WARPS * 32, 0, s>>>(
             bvh->d_nodes, had, bvh->d_leaves, parent_entries, d.n_tab[l], d.w[l], need,
+            (cut->flags & HCC_CUT_ALG3_DISCARD) && l + 1 < d.m ? 1u : 0u,
             cut->d_entry_node + d.ent_off[l], cut->d_table_cnt + d.tab_off[l],
             cut->d_boxes + 2 * (size_t)d.ent_off[l]);
     }
@@ -215,17 +221,25 @@ static int32_t set_levels(hcc_cut *cut, const uint32_t *widths, uint32_t m, uint
     cut->key_bits = key_bits;
     cut->container_bits = key_bits <= 32 ? 32u : 64u;
     cut->K_eff = (uint32_t)(nt);
+    cut->flags = 0u;
     cut->valid = true;
     return HCC_OK;
 }
 
-extern "C" int32_t hcc_select_cut_levels(const hcc_bvh *bvh, const float *density_dev, const uint32_t *widths,
-                                         uint32_t m, uint32_t key_bits, hcc_cut *cut, void *stream) {
+extern "C" int32_t hcc_select_cut_levels_ex(const hcc_bvh *bvh, const float *density_dev, const uint32_t *widths,
+                                            uint32_t m, uint32_t key_bits, uint32_t flags, hcc_cut *cut, void *stream) {
     HCC_REQUIRE(bvh && density_dev && widths && cut, HCC_ERR_INVALID_ARG, "hcc_select_cut: NULL argument");
     HCC_REQUIRE(aligned(density_dev, 16), HCC_ERR_BAD_ALIGNMENT, "hcc_select_cut: density_dev not 16-byte aligned");
+    HCC_REQUIRE((flags & ~(uint32_t)HCC_CUT_ALG3_DISCARD) == 0u, HCC_ERR_INVALID_ARG, "hcc_select_cut: unknown flags 0x%x", flags);
     int32_t rc = set_levels(cut, widths, m, key_bits);
     if (rc != HCC_OK) return rc;
+    cut->flags = flags;
     return launch_build_tables(bvh, density_dev, cut, (cudaStream_t)stream);
+}
+
+extern "C" int32_t hcc_select_cut_levels(const hcc_bvh *bvh, const float *density_dev, const uint32_t *widths,
+                                         uint32_t m, uint32_t key_bits, hcc_cut *cut, void *stream) {
+    return hcc_select_cut_levels_ex(bvh, density_dev, widths, m, key_bits, 0u, cut, stream);
 }
 
 // (f4) regular grid tables; the cell rule is stated in include/hcc.h

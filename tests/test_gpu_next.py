@@ -159,3 +159,28 @@ def test_reorder_trace_host_async_matches_the_device_path(hcc, cases):
         assert torch.equal(hits_b.cuda(), ref_b)
     ms = pa.stage_ms()
     assert ms["h2d"] > 0 and ms["trace"] > 0
+
+
+# ------------------------------------------------------------------ f4: Algorithm 3 as printed (discard)
+@pytest.mark.parametrize("name", ["tiny", "room_mid"])
+@pytest.mark.parametrize("widths,bits", [([8, 8], 16), ([16, 8, 8], 32), ([4, 4, 4], 16), ([16, 16, 16], 64), ([32], 32)])
+def test_alg3_discard_tables_and_keys_bit_exact(hcc, cases, name, widths, bits):
+    import oracle
+    d = cases[name]
+    b = d["case"].bvh
+    had = hcc.density(d["bvh"])
+    cut = hcc.select_cut_levels(d["bvh"], had, widths, bits, flags=hcc.CUT_ALG3_DISCARD)
+    want = oracle.level_tables(b.nodes, oracle.had(b.nodes), widths, discard=True)
+    ent, cnt = cut.read()
+    assert np.array_equal(cnt, want.table_cnt)
+    assert np.array_equal(ent, want.entry_node)
+    rays_h = d["case"].diffuse[:20011]
+    got = hcc.keys_to_numpy(hcc.encode(torch.from_numpy(rays_h).cuda(), cut)).astype(np.uint64)
+    assert np.array_equal(got, oracle.encode_hcc(rays_h, b.nodes, want))
+    # the flag is per selection: the same handle re-selected without it gives reading R4's tables again
+    hcc.select_cut_levels(d["bvh"], had, widths, bits, cut=cut)
+    ent2, cnt2 = cut.read()
+    kept = oracle.level_tables(b.nodes, oracle.had(b.nodes), widths)
+    assert np.array_equal(ent2, kept.entry_node) and np.array_equal(cnt2, kept.table_cnt)
+    with pytest.raises(hcc.HccError):
+        hcc.select_cut_levels(d["bvh"], had, widths, bits, flags=6)

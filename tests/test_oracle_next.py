@@ -183,3 +183,115 @@ def test_ppc_vs_recursive_walk_and_prefix_property(tiny, bits):
     root_hit = np.array([oracle.slab_hit(r, b.nodes["lo"][0], b.nodes["hi"][0]) for r in rays])
     assert np.array_equal((keys >> np.uint64(bits - 1)).astype(bool), root_hit)
     assert np.all(keys[~root_hit] == 0)
+
+
+# ------------------------------------------------------------------------------- f4: literal Algorithm 3
+def _leaf(x, k):
+    return ((x, 0, 0), (x + 0.5, 1, 1), k, 1)
+
+
+def test_alg3_discard_drops_a_popped_small_node():
+    """"we discard the top-level node that does not have a sufficient subtree (as shown in
+    line 6 of Algorithm 3)".  Hand tree: the root's left child is one big leaf with the highest HAD (so it
+    IS popped), its right child has 4 small leaves.  Level widths 3 x 2.
+      literal Alg. 3: pop root -> {1, 2}; pop 1: not large enough -> dropped; pop 2 -> {3, 4}; pop 3 -> {4, 5, 6}
+      reading R4    : pop root -> {1, 2}; pop 1 -> retired, MaxQueueSize 2; pop 2 -> {3, 4}: cut {1, 3, 4}"""
+    tris = np.zeros((5, 3, 3), np.float32)
+    small = lambda x, k: ((x, 0, 0), (x + 1.5, 1, 1), k, 1)
+    nodes = [((0, 0, 0), (7, 3, 3), 1, 0),        # 0 root
+             ((0, 0, 0), (3, 3, 3), 0, 1),         # 1 leaf, SA 54 -> HAD 54
+             ((4, 0, 0), (7, 1, 1), 3, 0),         # 2 internal, 4 leaves, HAD 35.75
+             ((4, 0, 0), (5.5, 1, 1), 5, 0),       # 3
+             ((5.5, 0, 0), (7, 1, 1), 7, 0),       # 4
+             small(4.0, 1), small(4.0, 2), small(5.5, 3), small(5.5, 4)]
+    b = hcc_inputs.make_bvh(nodes, tris)
+    had = oracle.had(b.nodes)
+    assert had[1] == 54.0 and had[2] == 35.75 and had[1] > had[2]
+    kept = oracle.level_tables(b.nodes, had, [3, 2])
+    lit = oracle.level_tables(b.nodes, had, [3, 2], discard=True)
+    assert sorted(kept.table(0, 0).tolist()) == [1, 3, 4]
+    assert sorted(lit.table(0, 0).tolist()) == [4, 5, 6]
+    assert np.array_equal(oracle.cut(b.nodes, had, 3, need=2, discard=True), lit.table(0, 0))
+    # what the literal variant gives up (the reason for reading R4): leaf 1 is under no level-1 entry,
+    # and entries 5, 6 (never popped) still get one-entry low tables, so :210's guarantee does not hold
+    parent = {1: 0, 2: 0, 3: 2, 4: 2, 5: 3, 6: 3, 7: 4, 8: 4}
+    covered = lambda leaf, cut: any(x in cut for x in (leaf, parent[leaf], parent.get(parent[leaf], -1)))
+    assert not covered(1, set(lit.table(0, 0).tolist())) and covered(1, set(kept.table(0, 0).tolist()))
+    ent = lit.level_entries(0).tolist()
+    assert len(lit.table(1, ent.index(5))) == 1 and len(lit.table(1, ent.index(4))) == 2
+
+
+@pytest.mark.parametrize("widths", [[8, 8], [16, 8, 8], [4, 4, 4]])
+def test_alg3_discard_properties_on_a_real_bvh(tiny, widths):
+    b = tiny.bvh
+    had = oracle.had(b.nodes)
+    leaves = oracle.subtree_leaves(b.nodes)
+    lit = oracle.level_tables(b.nodes, had, widths, discard=True)
+    kept = oracle.level_tables(b.nodes, had, widths)
+    m = len(widths)
+    for l in range(m - 1):
+        ent = lit.level_entries(l)
+        valid = ent[ent != 0xFFFFFFFF]
+        assert np.all(leaves[valid] >= 1)
+        # every kept entry of an upper level is either expandable-sized or was still queued when the loop ended;
+        # the tables below the large ones are full ("no empty low-level nodes")
+        for e, node in enumerate(ent):
+            if node != 0xFFFFFFFF and leaves[node] >= widths[l + 1]:
+                assert len(lit.table(l + 1, e)) == widths[l + 1] or l + 1 < m - 1
+    # the last level is Algorithm 2 in both variants: the table under entry e is Cut(node(e), w, need = 2)
+    parents = lit.level_entries(m - 2)
+    checked = 0
+    for e, node in enumerate(parents):
+        if node != 0xFFFFFFFF and checked < 25:
+            assert np.array_equal(lit.table(m - 1, e), oracle.cut(b.nodes, had, widths[m - 1], start=int(node), need=2))
+            checked += 1
+    # (with need = 8 on a 1,024-triangle scene the literal variant can drain its queue and leave whole
+    #  tables empty - the pathology DESIGN.md's reading R4 names; then there is nothing to check here)
+    assert checked > 0 or int((parents != 0xFFFFFFFF).sum()) == 0
+    # level 1 of the literal variant is Cut(root, w0, need = w1) with dropping, and never larger than w0
+    assert np.array_equal(lit.table(0, 0), oracle.cut(b.nodes, had, widths[0], need=widths[1], discard=True))
+    # dropping can only lose coverage: the leaves under the literal level-1 entries are a subset of all leaves,
+    # while reading R4's level 1 covers every leaf
+    assert leaves[lit.table(0, 0)].sum() <= leaves[kept.table(0, 0)].sum() == leaves[0]
+    # a single level has no level below it: the flag changes nothing
+    a = oracle.level_tables(b.nodes, had, [32], discard=True)
+    c = oracle.level_tables(b.nodes, had, [32])
+    assert np.array_equal(a.entry_node, c.entry_node)
+
+
+def test_alg3_discard_equals_retire_when_every_subtree_is_large():
+    """On a perfect tree cut well above the leaves no popped node is too small: both variants agree."""
+    depth = 7
+    n_nodes = 2 ** (depth + 1) - 1
+    # pre-order perfect binary tree with level-uniform boxes
+    nodes, tris = [None] * n_nodes, []
+    counter = [0]
+
+    def build(level, lo, hi):
+        i = counter[0]; counter[0] += 1
+        if level == depth:
+            nodes[i] = ((lo, 0, 0), (hi, 1, 1), len(tris), 1)
+            tris.append(np.zeros((3, 3), np.float32))
+            return i
+        nodes[i] = None
+        left = counter[0]
+        mid = 0.5 * (lo + hi)
+        build(level + 1, lo, mid)
+        build(level + 1, mid, hi)
+        nodes[i] = ((lo, 0, 0), (hi, 1, 1), left, 0)
+        return i
+    # children must be adjacent (right = left + 1): number breadth-first instead
+    nodes = []
+    width = 1
+    for level in range(depth + 1):
+        for k in range(width):
+            lo, hi = k / width, (k + 1) / width
+            idx = len(nodes)
+            first_child = (2 ** (level + 1) - 1) + 2 * k
+            nodes.append(((lo, 0, 0), (hi, 1, 1), first_child, 0) if level < depth else ((lo, 0, 0), (hi, 1, 1), k, 1))
+        width *= 2
+    b = hcc_inputs.make_bvh(nodes, np.zeros((2 ** depth, 3, 3), np.float32))
+    had = oracle.had(b.nodes)
+    a = oracle.level_tables(b.nodes, had, [4, 4], discard=True)
+    c = oracle.level_tables(b.nodes, had, [4, 4])
+    assert np.array_equal(a.entry_node, c.entry_node) and np.array_equal(a.table_cnt, c.table_cnt)
