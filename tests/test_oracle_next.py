@@ -1,6 +1,6 @@
 """Pins of the oracle functions behind the NEXT rows of the scope table:
 f1 sort truncation, f3 prefix path code (Figure 5),
-f4 regular grid encoding.  CPU only."""
+f4 regular grid encoding and Algorithm 3 as printed.  CPU only."""
 import os
 
 import numpy as np
