@@ -15,11 +15,11 @@ torch = pytest.importorskip("torch")
 SAMPLE = 4096
 
 
-def _run(hcc, name, bounce):
+def _run(hcc, name, bounce, res_scale=1.0):
     import hcc_inputs
     import oracle
     from hcc_inputs import rng as hrng
-    w = hcc_inputs.Workload(name)
+    w = hcc_inputs.Workload(name, res_scale=res_scale)
     b = w.bvh
     bvh = hcc.Bvh(b.nodes, b.tris, b.prim_idx)
 
@@ -94,3 +94,11 @@ def test_config3_full_size_second_bounce(hcc):
     """Config 3 (~1 M triangles, 1920x1080x8 spp, 64-bit keys 16x16x16), the rays of bounce 2."""
     n_d, n_s = _run(hcc, "fig1", 2)
     assert n_d > 16_000_000 and n_s > 32_000_000
+
+
+def test_config5_scene_in_full_at_quarter_resolution(hcc):
+    """Config 5's scene in full (10.8 M triangles, 7.1 M nodes: a BVH far larger than L2, traversal
+    stacks deeper than the 16 shared-memory entries) with 480x270x16 primaries: K = 16,384, 64-bit
+    keys 16x16x8x8."""
+    n_d, n_s = _run(hcc, "large", 1, res_scale=0.25)
+    assert n_d > 2_000_000 and n_s == 2 * n_d
