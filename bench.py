@@ -489,6 +489,18 @@ def run_ours(args):
                 sweep.append({"order": "hcc", "key_bits": kb, "K": K, "K_eff": i_s["K_eff"], "widths": i_s["widths"],
                               "bits_used": i_s["bits_used"], **run_order(hcc_keys(cut_s), i_s["bits_used"])})
         studies["sweep"] = sweep
+        # the same rays in a SHUFFLED input order (a wavefront renderer does not emit rays in camera order):
+        # the regime in which reordering has something to gain
+        saved = batches
+        g = torch.Generator(device="cuda").manual_seed(0x5EED)
+        batches = tuple((rays[torch.randperm(rays.shape[0], device="cuda", generator=g)].contiguous(), mode, name)
+                        for rays, mode, name in saved)
+        studies["orders_shuffled_input"] = {
+            "nosort": run_order(None, 0),
+            "twopoint": run_order(lambda rays, keys=None: hcc.encode_twopoint(rays, bvh.scene_lo, bvh.scene_hi, w.key_bits, keys=keys), tp_bits),
+            "hcc": run_order(hcc_keys(cut), info["bits_used"])}
+        batches = saved
+        step(hcc.ORDER_HCC)          # the hit buffers hold the unshuffled batches' results again (checked by the e2e leg)
         studies["note"] = ("per batch medians of 5; grid = regular-grid tables of the same widths through the same encoder; "
                            "ppc = prefix path code with key_bits tests (upper-bound ordering, PAPER.md:128)")
 
