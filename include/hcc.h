@@ -96,7 +96,8 @@ HCC_API int32_t hcc_version(void);
  * The BVH is INPUT (BASELINE.json north_star: built by a deterministic host binned-SAH
  * builder); the paper assumes a SAH BVH and does not describe a builder.
  * hcc_bvh_create validates the canonical arrays on the host (indices in range, siblings
- * adjacent, parent < child, every node reachable once, leaf count in 1..8, depth <= 63:
+ * adjacent, parent < child, every node reachable once, leaf count in 1..8, depth <= 63,
+ * fewer than 2^27 triangles and 2^30 nodes:
  * otherwise HCC_ERR_INVALID_ARG / HCC_ERR_UNSUPPORTED), copies them to the device and runs
  * the conversion kernels on `stream`: one 32-byte traversal record per internal node
  * (both child boxes as 15-bit cells of a uniform grid over the root box, rounded outwards
@@ -246,7 +247,11 @@ HCC_API int32_t hcc_sort_range(void *keys_dev, uint64_t n, uint32_t container_bi
  * Rays are traced in the order perm_dev[0], perm_dev[1], ... (perm_dev == NULL: 0, 1, ...,
  * the NoSort order): warps take consecutive 32-rank chunks of that order, and every result
  * is written at the ray's own index ("the trace kernel fetches the rays based
- * on these sorted indices").  CLOSEST: hits_dev = hcc_hit[n]: the triangle with the
+ * on these sorted indices").  n < 2^32 - 2^24.  Up to 1024 trace launches on one hcc_bvh may
+ * be in flight at a time (each takes its own work counter, zeroed on `stream`).  The quantised
+ * boxes are tested with a slack proportional to the distance of the ray origin from the scene
+ * (2^-20 of it), which covers the fp32 rounding of the plane distances for origins up to about
+ * 10^4 scene extents away; beyond that a triangle may be culled that the predicate would accept.  CLOSEST: hits_dev = hcc_hit[n]: the triangle with the
  * smallest t in (tmin, tmax), ties to the lowest prim id.  ANY: hits_dev = uint8[n].
  * Triangle test (fp32, fmaf where written): e1 = v1-v0, e2 = v2-v0, p = d x e2,
  * det = e1.p (0 -> miss), inv = 1/det, s = o-v0, u = (s.p)*inv, q = s x e1, v = (d.q)*inv,
@@ -255,9 +260,13 @@ HCC_API int32_t hcc_sort_range(void *keys_dev, uint64_t n, uint32_t container_bi
 HCC_API int32_t hcc_trace(const hcc_bvh *bvh, const float *rays_dev, uint64_t n, const uint32_t *perm_dev,
                   int32_t mode, void *hits_dev, void *stream);
 
-/* Same traversal, instrumented (never used for timing): stats_dev = uint64[4], zeroed by the
- * call, then [0] = sibling-pair records fetched (32 bytes each), [1] = triangle records fetched
- * (64 bytes each), [2] = rays traced, [3] = deepest traversal stack.  hits_dev as hcc_trace. */
+/* Same traversal, instrumented (never used for timing): stats_dev = uint64[8], zeroed by the
+ * call, then [0] = sibling-pair records fetched by rays (32 bytes each), [1] = triangle records
+ * fetched (64 bytes each), [2] = rays traced, [3] = deepest traversal stack, and per WARP-level
+ * node step (the 32 rays a warp holds fetch their records with one load instruction): [4] =
+ * distinct records fetched, summed over steps, [5] = steps, [6] = lanes taking part, summed.
+ * [4]/[5] is what a coherent order lowers (rays of a warp sharing node
+ * fetches); [0] does not depend on the order.  [7] is reserved.  hits_dev as hcc_trace. */
 HCC_API int32_t hcc_trace_stats(const hcc_bvh *bvh, const float *rays_dev, uint64_t n, const uint32_t *perm_dev,
                         int32_t mode, void *hits_dev, uint64_t *stats_dev, void *stream);
 

@@ -14,7 +14,8 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libhcc_b200.so")
+# HCC_B200_LIB names another build of the same library (kernel tuning variants); default: the in-tree one
+LIB_PATH = os.environ.get("HCC_B200_LIB") or os.path.join(_HERE, "libhcc_b200.so")
 
 MISS_PRIM = 0xFFFFFFFF
 MAX_LEVELS = 16
@@ -334,17 +335,20 @@ def keys_to_numpy(keys):
 
 
 def trace_stats(bvh, rays, perm=None, mode=TRACE_CLOSEST, stream=None):
-    """hcc_trace_stats: dict(pairs, tris, rays, max_stack, node_bytes_per_ray, tri_bytes_per_ray)."""
+    """hcc_trace_stats: dict(pairs, tris, rays, max_stack, node_bytes_per_ray, tri_bytes_per_ray, and per
+    warp-level node step: distinct pair records (sectors_per_step) and lanes taking part (lanes_per_step))."""
     n = rays.shape[0]
     hits = (torch.empty((n, 4), dtype=torch.float32, device="cuda") if mode == TRACE_CLOSEST
             else torch.empty(n, dtype=torch.uint8, device="cuda"))
-    st = torch.zeros(4, dtype=torch.int64, device="cuda")
+    st = torch.zeros(8, dtype=torch.int64, device="cuda")
     p = _vp(0) if perm is None else _dev(perm, (torch.int32,), "perm")
     _check(lib().hcc_trace_stats(bvh._h, _rays_dev(rays), n, p, int(mode), _vp(hits.data_ptr()),
                                  _vp(st.data_ptr()), _stream(stream)))
-    pairs, tris, nr, depth = [int(x) for x in st.cpu().tolist()]
+    pairs, tris, nr, depth, sectors, steps, lanes, _ = [int(x) for x in st.cpu().tolist()]
     return dict(pairs=pairs, tris=tris, rays=nr, max_stack=depth,
-                node_bytes_per_ray=32.0 * pairs / max(nr, 1), tri_bytes_per_ray=64.0 * tris / max(nr, 1))
+                node_bytes_per_ray=32.0 * pairs / max(nr, 1), tri_bytes_per_ray=64.0 * tris / max(nr, 1),
+                warp_steps=steps, sectors_per_step=sectors / max(steps, 1), lanes_per_step=lanes / max(steps, 1),
+                distinct_node_bytes_per_ray=32.0 * sectors / max(nr, 1))
 
 
 def anc(keys, perm=None, stream=None):

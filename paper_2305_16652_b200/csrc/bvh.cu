@@ -166,8 +166,8 @@ extern "C" int32_t hcc_bvh_create(const hcc_node *nodes, uint32_t n_nodes, const
                                   const uint32_t *prim_idx, void *stream, hcc_bvh **out) {
     HCC_REQUIRE(nodes && tris && prim_idx && out, HCC_ERR_INVALID_ARG, "hcc_bvh_create: NULL argument");
     HCC_REQUIRE(n_nodes >= 1 && n_tris >= 1, HCC_ERR_INVALID_ARG, "hcc_bvh_create: empty BVH");
-    HCC_REQUIRE(n_tris < (1u << 28) && n_nodes < (1u << 30), HCC_ERR_UNSUPPORTED,
-                "hcc_bvh_create: more than 2^28 triangles or 2^30 nodes");
+    HCC_REQUIRE(n_tris < (1u << 27) && n_nodes < (1u << 30), HCC_ERR_UNSUPPORTED,
+                "hcc_bvh_create: more than 2^27 triangles or 2^30 nodes");
     *out = nullptr;
     cudaStream_t s = (cudaStream_t)stream;
 
@@ -234,7 +234,7 @@ extern "C" int32_t hcc_bvh_create(const hcc_node *nodes, uint32_t n_nodes, const
     alloc((void **)&b->d_flags, sizeof(uint32_t) * (size_t)n_nodes);
     alloc((void **)&b->d_internal, sizeof(uint32_t) * (internal_ids.size() + 1));
     alloc((void **)&b->d_qrec, 32 * (internal_ids.size() + 1));
-    alloc((void **)&b->d_trace_ctl, 2 * 256 * sizeof(uint32_t));
+    alloc((void **)&b->d_trace_ctl, 2 * HCC_TRACE_SLOTS * sizeof(uint32_t));
     alloc((void **)&b->d_ttri, sizeof(float4) * 4 * (size_t)n_tris);
     alloc((void **)&d_rank, sizeof(uint32_t) * (size_t)n_nodes);
     alloc((void **)&d_tris, sizeof(float) * 9 * (size_t)n_tris);
@@ -258,7 +258,7 @@ extern "C" int32_t hcc_bvh_create(const hcc_node *nodes, uint32_t n_nodes, const
     if (!internal_ids.empty() &&
         (e = cudaMemcpyAsync(b->d_internal, internal_ids.data(), sizeof(uint32_t) * internal_ids.size(), cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy internal ids");
     if ((e = cudaMemsetAsync(b->d_flags, 0, sizeof(uint32_t) * (size_t)n_nodes, s)) != cudaSuccess) return fail(e, "memset");
-    if ((e = cudaMemsetAsync(b->d_trace_ctl, 0, 2 * 256 * sizeof(uint32_t), s)) != cudaSuccess) return fail(e, "memset");
+    if ((e = cudaMemsetAsync(b->d_trace_ctl, 0, 2 * HCC_TRACE_SLOTS * sizeof(uint32_t), s)) != cudaSuccess) return fail(e, "memset");
     const uint32_t T = 256;
     k_parents<<<(n_nodes + T - 1) / T, T, 0, s>>>(b->d_nodes, n_nodes, b->d_parent);
     if (b->n_internal)

@@ -50,6 +50,10 @@ inline uint64_t round_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
 constexpr float HCC_GRID_CELLS = 32763.0f;
 constexpr float HCC_GRID_OFFSET = 2.0f;
 constexpr uint32_t HCC_REF_LEAF = 0x80000000u;
+// Extra slack of the traversal's slab test, as a fraction of (|ray origin in cells| + 65536): 2^-20,
+// about four times the rounding of the fp32 plane distances (trace.cu).
+constexpr float HCC_TRACE_PAD = 9.5367431640625e-07f;
+constexpr int HCC_TRACE_SLOTS = 1024;   // work counters of trace launches in flight on one BVH
 
 // Device-side level tables of a cut hierarchy, passed to kernels by value.
 struct CutDev {
@@ -80,7 +84,7 @@ struct hcc_bvh {
     float4 *d_ttri;         // 4 float4 (64 bytes) per triangle, leaf order
     uint32_t n_internal;
     uint32_t root_ref;      // traversal reference of the root (see bvh.cu)
-    uint32_t *d_trace_ctl;  // 256 x {next rank, CTAs done}: work counters of trace launches in flight
+    uint32_t *d_trace_ctl;  // HCC_TRACE_SLOTS x {next rank, -}: work counters of trace launches in flight
     std::atomic<uint32_t> *trace_calls;
     float q_lo[3], q_scale[3];   // traversal grid: g = (x - q_lo) * q_scale + HCC_GRID_OFFSET
     // scratch for hcc_select_cut_flat lives in the caller's workspace

@@ -421,6 +421,47 @@ def test_trace_axis_parallel_rays_vs_brute_force(hcc, tiny):
     assert (~np.isinf(want[0])).sum() > 50
 
 
+@pytest.mark.parametrize("dist", [30.0, 1000.0, 5000.0])
+def test_trace_distant_origins_vs_brute_force(hcc, tiny, dist):
+    """Origins `dist` scene extents away, aimed at points inside the scene: the slack of the
+    quantised slab test grows with the origin's distance (include/hcc.h, hcc_trace), so no box
+    holding a triangle the predicate accepts is culled.  (The triangle predicate itself is
+    evaluated with the same coarse fp32 origin on both sides.)"""
+    from hcc_inputs import rng as hrng
+    n = 4000 + 7
+    u = hrng.u01(0xFA4, int(dist), np.arange(n, dtype=np.uint64), np.arange(6, dtype=np.uint64)[:, None]).T
+    target = (0.1 + 0.8 * u[:, 0:3]).astype(np.float32)
+    d = 2.0 * u[:, 3:6] - 1.0
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    rays = np.zeros((n, 8), dtype=np.float32)
+    rays[:, 0:3] = target - np.float32(dist) * d.astype(np.float32)
+    o = rays[:, 0:3].astype(np.float64)
+    dd = target.astype(np.float64) - o                      # direction recomputed from the ROUNDED origin
+    dd /= np.linalg.norm(dd, axis=1, keepdims=True)
+    rays[:, 4:7] = dd
+    rays[:, 3] = 0.0
+    rays[:, 7] = np.inf
+    want = _check_trace_both_modes(hcc, tiny.bvh, rays)
+    assert (~np.isinf(want[0])).sum() > 50
+
+
+def test_trace_many_launches_in_flight_on_two_streams(hcc, dev_cases):
+    """More launches than work-counter slots (1024), alternating between two streams: every launch
+    zeroes its own counter on its own stream, so results never depend on what ran before."""
+    d = dev_cases["room_small"]
+    ref = hcc.trace(d["bvh"], d["diffuse"], None, hcc.TRACE_CLOSEST)
+    sub = d["diffuse"][:999].contiguous()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs = [torch.empty((999, 4), dtype=torch.float32, device="cuda") for _ in range(2)]
+    torch.cuda.synchronize()
+    for i in range(1100):
+        with torch.cuda.stream(streams[i & 1]):
+            hcc.trace(d["bvh"], sub, None, hcc.TRACE_CLOSEST, hits=outs[i & 1], stream=streams[i & 1])
+    torch.cuda.synchronize()
+    for o in outs:
+        assert torch.equal(o.view(torch.int32), ref[:999].view(torch.int32))
+
+
 def test_trace_flat_scene_vs_brute_force(hcc):
     """All triangles in the plane z = 0.25 (zero scene extent along z): the traversal grid is
     degenerate on that axis."""
