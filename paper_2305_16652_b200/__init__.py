@@ -335,8 +335,9 @@ def keys_to_numpy(keys):
 
 
 def trace_stats(bvh, rays, perm=None, mode=TRACE_CLOSEST, stream=None):
-    """hcc_trace_stats: dict(pairs, tris, rays, max_stack, node_bytes_per_ray, tri_bytes_per_ray, and per
-    warp-level node step: distinct pair records (sectors_per_step) and lanes taking part (lanes_per_step))."""
+    """hcc_trace_stats: dict(nodes, tris, rays, max_stack, node_bytes_per_ray, tri_bytes_per_ray; per warp-level
+    node step: distinct node records (records_per_step) and lanes taking part (lanes_per_step); per warp-level
+    triangle round: lanes busy (lanes_per_tri_round))."""
     n = rays.shape[0]
     hits = (torch.empty((n, 4), dtype=torch.float32, device="cuda") if mode == TRACE_CLOSEST
             else torch.empty(n, dtype=torch.uint8, device="cuda"))
@@ -344,11 +345,12 @@ def trace_stats(bvh, rays, perm=None, mode=TRACE_CLOSEST, stream=None):
     p = _vp(0) if perm is None else _dev(perm, (torch.int32,), "perm")
     _check(lib().hcc_trace_stats(bvh._h, _rays_dev(rays), n, p, int(mode), _vp(hits.data_ptr()),
                                  _vp(st.data_ptr()), _stream(stream)))
-    pairs, tris, nr, depth, sectors, steps, lanes, _ = [int(x) for x in st.cpu().tolist()]
-    return dict(pairs=pairs, tris=tris, rays=nr, max_stack=depth,
-                node_bytes_per_ray=32.0 * pairs / max(nr, 1), tri_bytes_per_ray=64.0 * tris / max(nr, 1),
-                warp_steps=steps, sectors_per_step=sectors / max(steps, 1), lanes_per_step=lanes / max(steps, 1),
-                distinct_node_bytes_per_ray=32.0 * sectors / max(nr, 1))
+    nodes, tris, nr, depth, records, steps, lanes, rounds = [int(x) for x in st.cpu().tolist()]
+    return dict(nodes=nodes, tris=tris, rays=nr, max_stack=depth,
+                node_bytes_per_ray=64.0 * nodes / max(nr, 1), tri_bytes_per_ray=64.0 * tris / max(nr, 1),
+                warp_steps=steps, records_per_step=records / max(steps, 1), lanes_per_step=lanes / max(steps, 1),
+                distinct_node_bytes_per_ray=64.0 * records / max(nr, 1),
+                tri_rounds=rounds, lanes_per_tri_round=tris / max(rounds, 1))
 
 
 def anc(keys, perm=None, stream=None):

@@ -25,12 +25,15 @@ void set_error(const char *fmt, ...) {
 
 // Traversal records.  Nothing on the results depends on them: the hit a ray reports is defined
 // by the triangle predicate alone (include/hcc.h), box culling only has to be conservative.
-// So the child boxes are stored compactly: the k-th INTERNAL node (node order) owns one
-// 32-byte record holding BOTH children, fetched with one 256-bit load per traversal step:
-//   w[0..2] = left child x, y, z:  lo cell | hi cell << 16     w[3..5] = right child
-//   w[6], w[7] = left, right child reference
-//   reference, internal child: (rank of the child among internal nodes) + 1      (bit 31 clear)
+// The binary BVH is collapsed on the host into a 4-wide one (hcc_bvh_create: starting from a
+// node's two children, the internal child with the largest surface area is replaced by its own
+// two children until there are four or only leaves are left), so a ray makes about half as many
+// dependent record fetches.  The k-th WIDE node owns one 64-byte record, two 256-bit loads:
+//   w[3c .. 3c+2] = child c (0..3) x, y, z:  lo cell | hi cell << 16
+//   w[12 + c]     = reference of child c
+//   reference, internal child: (index of its wide node) + 1                       (bit 31 clear)
 //   reference, leaf child    : 0x80000000 | (count-1) << 28 | first triangle slot
+//   unused slot              : reference 0, box lo cell 32767 / hi cell 0 (never hit)
 // Cells are indices of a uniform grid over the root box, g = (x - q_lo) * q_scale + 2 in fp32
 // (a monotone map, so containment survives it), lo = floor(g) - 1, hi = ceil(g) + 1, clamped to
 // [0, 32767]: every stored box contains the fp32 box with a margin of at least one cell
@@ -48,19 +51,24 @@ __global__ void k_parents(const hcc_node *__restrict__ nodes, uint32_t n, uint32
 
 struct GridFrame { float lo[3], scale[3]; };
 
-__device__ __forceinline__ uint32_t node_ref(const hcc_node &nd, uint32_t rank) {
-    return nd.count == 0 ? rank + 1u : (HCC_REF_LEAF | ((nd.count - 1u) << 28) | nd.left_or_first);
-}
+constexpr uint32_t WIDE_NONE = 0xFFFFFFFFu;
 
-__global__ void k_build_qrec(const hcc_node *__restrict__ nodes, const uint32_t *__restrict__ internal,
-                             const uint32_t *__restrict__ rank, uint32_t n_internal, GridFrame f,
-                             uint32_t *__restrict__ qrec) {
+// wchild: 4 binary node ids per wide node (WIDE_NONE = unused slot); wide_of: wide node index of a
+// binary node that heads a wide node.
+__global__ void k_build_wrec(const hcc_node *__restrict__ nodes, const uint32_t *__restrict__ wchild,
+                             const uint32_t *__restrict__ wide_of, uint32_t n_wide, GridFrame f,
+                             uint32_t *__restrict__ wrec) {
     uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= n_internal) return;
-    const uint32_t left = nodes[internal[k]].left_or_first;
-    uint32_t w[8];
-    for (uint32_t c = 0; c < 2; ++c) {
-        const hcc_node ch = nodes[left + c];
+    if (k >= n_wide) return;
+    uint32_t w[16];
+    for (uint32_t c = 0; c < 4; ++c) {
+        const uint32_t id = wchild[4 * (size_t)k + c];
+        if (id == WIDE_NONE) {
+            w[3 * c] = w[3 * c + 1] = w[3 * c + 2] = 0x00007FFFu;
+            w[12 + c] = 0u;
+            continue;
+        }
+        const hcc_node ch = nodes[id];
         for (int a = 0; a < 3; ++a) {
             const float gl = (ch.lo[a] - f.lo[a]) * f.scale[a] + HCC_GRID_OFFSET;
             const float gh = (ch.hi[a] - f.lo[a]) * f.scale[a] + HCC_GRID_OFFSET;
@@ -70,11 +78,10 @@ __global__ void k_build_qrec(const hcc_node *__restrict__ nodes, const uint32_t 
             if (!(gl == gl) || !(gh == gh)) { ql = 0; qh = 32767; }
             w[3 * c + a] = (uint32_t)ql | ((uint32_t)qh << 16);
         }
-        w[6 + c] = node_ref(ch, rank[left + c]);
+        w[12 + c] = ch.count == 0 ? wide_of[id] + 1u : (HCC_REF_LEAF | ((ch.count - 1u) << 28) | ch.left_or_first);
     }
-    uint4 *out = reinterpret_cast<uint4 *>(qrec + 8 * (size_t)k);
-    out[0] = make_uint4(w[0], w[1], w[2], w[3]);
-    out[1] = make_uint4(w[4], w[5], w[6], w[7]);
+    uint4 *out = reinterpret_cast<uint4 *>(wrec + 16 * (size_t)k);
+    for (int q = 0; q < 4; ++q) out[q] = make_uint4(w[4 * q], w[4 * q + 1], w[4 * q + 2], w[4 * q + 3]);
 }
 
 // Triangle record k (leaf order), 64 bytes so that it is two aligned 256-bit loads:
@@ -154,7 +161,7 @@ extern "C" int32_t hcc_bvh_destroy(hcc_bvh *b) {
     cudaFree(b->d_leaves);
     cudaFree(b->d_flags);
     cudaFree(b->d_internal);
-    cudaFree(b->d_qrec);
+    cudaFree(b->d_wrec);
     cudaFree(b->d_trace_ctl);
     delete b->trace_calls;
     cudaFree(b->d_ttri);
@@ -221,11 +228,52 @@ extern "C" int32_t hcc_bvh_create(const hcc_node *nodes, uint32_t n_nodes, const
     b->n_internal = (uint32_t)internal_ids.size();
     b->trace_calls = new std::atomic<uint32_t>(0u);
     b->root_ref = nodes[0].count == 0 ? 1u : (HCC_REF_LEAF | ((nodes[0].count - 1u) << 28) | nodes[0].left_or_first);
-    std::vector<uint32_t> rank(n_nodes, 0u);     // rank of an internal node among the internal nodes
-    for (uint32_t k = 0; k < b->n_internal; ++k) rank[internal_ids[k]] = k;
+
+    // ---- collapse to a 4-wide tree (host, one pass): wide node ids are handed out family by family
+    //      (the internal children of one wide node are neighbours) in depth-first order
+    std::vector<uint32_t> wide_of(n_nodes, WIDE_NONE), wchild;
+    {
+        auto area = [&](uint32_t i) {
+            const hcc_node &nd = nodes[i];
+            const float dx = nd.hi[0] - nd.lo[0], dy = nd.hi[1] - nd.lo[1], dz = nd.hi[2] - nd.lo[2];
+            return dx * dy + dy * dz + dz * dx;
+        };
+        std::vector<uint32_t> todo;        // binary nodes heading a wide node whose children are not yet chosen
+        uint32_t n_wide = 0;
+        if (nodes[0].count == 0) { wide_of[0] = n_wide++; todo.push_back(0u); }
+        wchild.reserve(4 * (size_t)(n_nodes / 3 + 2));
+        while (!todo.empty()) {
+            const uint32_t head = todo.back();
+            todo.pop_back();
+            uint32_t c[4] = {nodes[head].left_or_first, nodes[head].left_or_first + 1u, WIDE_NONE, WIDE_NONE};
+            uint32_t nc = 2;
+            while (nc < 4) {
+                int pick = -1;
+                float best = -1.0f;
+                for (uint32_t k = 0; k < nc; ++k)
+                    if (nodes[c[k]].count == 0) {
+                        const float a = area(c[k]);
+                        if (pick < 0 || a > best) { pick = (int)k; best = a; }
+                    }
+                if (pick < 0) break;
+                const uint32_t l = nodes[c[pick]].left_or_first;
+                c[pick] = l;
+                c[nc++] = l + 1u;
+            }
+            const size_t at = 4 * (size_t)wide_of[head];
+            if (wchild.size() < at + 4) wchild.resize(at + 4, WIDE_NONE);
+            for (uint32_t k = 0; k < 4; ++k) wchild[at + k] = c[k];
+            for (uint32_t k = 0; k < nc; ++k)
+                if (nodes[c[k]].count == 0) wide_of[c[k]] = n_wide++;
+            for (uint32_t k = nc; k-- > 0;)
+                if (nodes[c[k]].count == 0) todo.push_back(c[k]);
+        }
+        wchild.resize(4 * (size_t)n_wide, WIDE_NONE);
+        b->n_wide = n_wide;
+    }
 
     float *d_tris = nullptr;
-    uint32_t *d_prim = nullptr, *d_rank = nullptr;
+    uint32_t *d_prim = nullptr, *d_wide_of = nullptr, *d_wchild = nullptr;
     cudaError_t e = cudaSuccess;
     auto alloc = [&](void **p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
     alloc((void **)&b->d_nodes, sizeof(hcc_node) * (size_t)n_nodes);
@@ -233,43 +281,47 @@ extern "C" int32_t hcc_bvh_create(const hcc_node *nodes, uint32_t n_nodes, const
     alloc((void **)&b->d_leaves, sizeof(uint32_t) * (size_t)n_nodes);
     alloc((void **)&b->d_flags, sizeof(uint32_t) * (size_t)n_nodes);
     alloc((void **)&b->d_internal, sizeof(uint32_t) * (internal_ids.size() + 1));
-    alloc((void **)&b->d_qrec, 32 * (internal_ids.size() + 1));
+    alloc((void **)&b->d_wrec, 64 * ((size_t)b->n_wide + 1));
     alloc((void **)&b->d_trace_ctl, 2 * HCC_TRACE_SLOTS * sizeof(uint32_t));
     alloc((void **)&b->d_ttri, sizeof(float4) * 4 * (size_t)n_tris);
-    alloc((void **)&d_rank, sizeof(uint32_t) * (size_t)n_nodes);
+    alloc((void **)&d_wide_of, sizeof(uint32_t) * (size_t)n_nodes);
+    alloc((void **)&d_wchild, sizeof(uint32_t) * (wchild.size() + 4));
     alloc((void **)&d_tris, sizeof(float) * 9 * (size_t)n_tris);
     alloc((void **)&d_prim, sizeof(uint32_t) * (size_t)n_tris);
     if (e != cudaSuccess) {
         set_error("hcc_bvh_create: cudaMalloc failed: %s", cudaGetErrorString(e));
-        cudaFree(d_tris); cudaFree(d_prim); cudaFree(d_rank);
+        cudaFree(d_tris); cudaFree(d_prim); cudaFree(d_wide_of); cudaFree(d_wchild);
         hcc_bvh_destroy(b);
         return e == cudaErrorMemoryAllocation ? HCC_ERR_OUT_OF_MEMORY : HCC_ERR_CUDA;
     }
     auto fail = [&](cudaError_t err, const char *what) {
         set_error("hcc_bvh_create: %s: %s", what, cudaGetErrorString(err));
-        cudaFree(d_tris); cudaFree(d_prim); cudaFree(d_rank);
+        cudaFree(d_tris); cudaFree(d_prim); cudaFree(d_wide_of); cudaFree(d_wchild);
         hcc_bvh_destroy(b);
         return (int32_t)HCC_ERR_CUDA;
     };
     if ((e = cudaMemcpyAsync(b->d_nodes, nodes, sizeof(hcc_node) * (size_t)n_nodes, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy nodes");
     if ((e = cudaMemcpyAsync(d_tris, tris, sizeof(float) * 9 * (size_t)n_tris, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy triangles");
     if ((e = cudaMemcpyAsync(d_prim, prim_idx, sizeof(uint32_t) * (size_t)n_tris, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy prim_idx");
-    if ((e = cudaMemcpyAsync(d_rank, rank.data(), sizeof(uint32_t) * (size_t)n_nodes, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy ranks");
+    if ((e = cudaMemcpyAsync(d_wide_of, wide_of.data(), sizeof(uint32_t) * (size_t)n_nodes, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy wide ids");
+    if (!wchild.empty() &&
+        (e = cudaMemcpyAsync(d_wchild, wchild.data(), sizeof(uint32_t) * wchild.size(), cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy wide children");
     if (!internal_ids.empty() &&
         (e = cudaMemcpyAsync(b->d_internal, internal_ids.data(), sizeof(uint32_t) * internal_ids.size(), cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy internal ids");
     if ((e = cudaMemsetAsync(b->d_flags, 0, sizeof(uint32_t) * (size_t)n_nodes, s)) != cudaSuccess) return fail(e, "memset");
     if ((e = cudaMemsetAsync(b->d_trace_ctl, 0, 2 * HCC_TRACE_SLOTS * sizeof(uint32_t), s)) != cudaSuccess) return fail(e, "memset");
     const uint32_t T = 256;
     k_parents<<<(n_nodes + T - 1) / T, T, 0, s>>>(b->d_nodes, n_nodes, b->d_parent);
-    if (b->n_internal)
-        k_build_qrec<<<(b->n_internal + T - 1) / T, T, 0, s>>>(b->d_nodes, b->d_internal, d_rank, b->n_internal, frame, b->d_qrec);
+    if (b->n_wide)
+        k_build_wrec<<<(b->n_wide + T - 1) / T, T, 0, s>>>(b->d_nodes, d_wchild, d_wide_of, b->n_wide, frame, b->d_wrec);
     k_convert_tris<<<(n_tris + T - 1) / T, T, 0, s>>>(d_tris, d_prim, n_tris, b->d_ttri);
     k_subtree_leaves<<<(n_nodes + T - 1) / T, T, 0, s>>>(b->d_nodes, b->d_parent, b->d_flags, n_nodes, b->d_leaves);
     if ((e = cudaGetLastError()) != cudaSuccess) return fail(e, "conversion kernels");
     if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return fail(e, "synchronise");
     cudaFree(d_tris);
     cudaFree(d_prim);
-    cudaFree(d_rank);
+    cudaFree(d_wide_of);
+    cudaFree(d_wchild);
     *out = b;
     return HCC_OK;
 }

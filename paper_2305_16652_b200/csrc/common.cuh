@@ -80,7 +80,8 @@ struct hcc_bvh {
     uint32_t *d_leaves;     // sub-tree leaf counts
     uint32_t *d_flags;      // arrival counters of the bottom-up passes
     uint32_t *d_internal;   // indices of the internal nodes, ascending
-    uint32_t *d_qrec;       // traversal records: 8 words (32 bytes) per INTERNAL node, in node order
+    uint32_t *d_wrec;       // traversal records: 16 words (64 bytes) per node of the 4-wide tree (bvh.cu)
+    uint32_t n_wide;
     float4 *d_ttri;         // 4 float4 (64 bytes) per triangle, leaf order
     uint32_t n_internal;
     uint32_t root_ref;      // traversal reference of the root (see bvh.cu)

@@ -3,37 +3,44 @@
 //
 // Design: persistent warps pull 32-ray chunks of the (sorted) order from an
 // atomic counter and refill finished lanes from the same chunk, so the rays of a warp stay
-// neighbours in the sorted order; each traversal step fetches ONE 32-byte record holding both
-// quantised child boxes (bvh.cu) with a 256-bit load; the warp alternates between a node phase
-// and a triangle phase, each running while at least half of the live lanes take part (a
-// thresholded while-while loop); the stack lives in shared memory (conflict-free, 16 deep) and
-// spills to local memory below that.  Compiled with -fmad=false; fmaf() appears exactly where
-// hcc.h states it for the triangle predicate, which alone defines the results.
+// neighbours in the sorted order.  The warp alternates between two phases:
+//  - node phase: every lane that holds an internal reference fetches ONE 64-byte record of the
+//    4-wide tree (bvh.cu: four quantised child boxes + four references, two 256-bit loads), tests
+//    the four boxes, descends into the nearest hit child and pushes the others; it runs while at
+//    least half of the live lanes take part;
+//  - triangle phase: the leaves the lanes hold are flattened into (ray, triangle) items and the
+//    WHOLE warp tests 32 items per round, whoever owns the rays: the ray of an item is read from
+//    shared memory, a hit is committed to the owner's slot with a 64-bit shared-memory atomicMin
+//    on (t, prim) (closest hit) or a flag store (any hit).
+// The traversal stack lives in shared memory (conflict-free) and spills to local memory.
+// Compiled with -fmad=false; fmaf() appears exactly where hcc.h states it for the triangle
+// predicate, which alone defines the results.
 #include "common.cuh"
 
 namespace hcc {
 
 constexpr int TRACE_THREADS = 128;
-#ifndef HCC_TRACE_BLOCKS_PER_SM       // closest hit: 8 CTAs of 128 threads per SM (64 registers)
+#ifndef HCC_TRACE_BLOCKS_PER_SM       // closest hit: CTAs of 128 threads per SM
 #define HCC_TRACE_BLOCKS_PER_SM 8
 #endif
-#ifndef HCC_TRACE_BLOCKS_PER_SM_ANY   // any hit carries no (t, u, v, prim): 9 CTAs per SM (56 registers)
-#define HCC_TRACE_BLOCKS_PER_SM_ANY 9
+#ifndef HCC_TRACE_BLOCKS_PER_SM_ANY
+#define HCC_TRACE_BLOCKS_PER_SM_ANY 8
 #endif
 #ifndef HCC_TRACE_REFILL_AT
 #define HCC_TRACE_REFILL_AT 8
 #endif
-#ifndef HCC_TRACE_CLOSEST_STEPWISE   // closest-hit triangle phase: 1 = one triangle per lane per iteration, thresholded
-#define HCC_TRACE_CLOSEST_STEPWISE 0
+#ifndef HCC_TRACE_SMEM_STACK
+#define HCC_TRACE_SMEM_STACK 12
 #endif
-#ifndef HCC_TRACE_TRI_DEN            // triangle phase goes on while 1/TRI_DEN of the live lanes hold a leaf
-#define HCC_TRACE_TRI_DEN 4
+#ifndef HCC_TRACE_NODE_DEN            // node phase goes on while 1/NODE_DEN of the live lanes hold an internal reference
+#define HCC_TRACE_NODE_DEN 2
 #endif
 constexpr int TRACE_BLOCKS_PER_SM = HCC_TRACE_BLOCKS_PER_SM, TRACE_BLOCKS_PER_SM_ANY = HCC_TRACE_BLOCKS_PER_SM_ANY;
-constexpr int SMEM_STACK = 16;          // entries per thread in shared memory
-constexpr int STACK_SIZE = 64;          // hcc_bvh_create admits depth <= 63
+constexpr int SMEM_STACK = HCC_TRACE_SMEM_STACK;   // entries per thread in shared memory
+constexpr int STACK_SIZE = 3 * 63 + 4;  // hcc_bvh_create admits depth <= 63; a 4-wide step pushes at most 3
 constexpr uint32_t CHUNK = 32;          // rays a warp takes from the counter at a time
 constexpr uint32_t REFILL_AT = HCC_TRACE_REFILL_AT;   // idle lanes that trigger a refill
+constexpr int TRACE_WARPS = TRACE_THREADS / 32;
 
 __device__ __forceinline__ float max3(float a, float b, float c) {
     float d;
@@ -76,65 +83,76 @@ __device__ __forceinline__ uint32_t ld_stream(const uint32_t *p) {
     return r;
 }
 
-struct Ray {
-    float ox, oy, oz, tmin, dx, dy, dz, tmax;
-};
+// float bits <-> unsigned keys of the same order (negative t included)
+__device__ __forceinline__ uint32_t ord_of(float f) {
+    const uint32_t b = __float_as_uint(f);
+    return b ^ ((uint32_t)((int32_t)b >> 31) | 0x80000000u);
+}
+__device__ __forceinline__ float float_of(uint32_t k) {
+    return __uint_as_float(k ^ (((k >> 31) - 1u) | 0x80000000u));
+}
 
-// The triangle predicate of hcc.h, operation by operation.
-__device__ __forceinline__ bool tri_hit(const Ray &r, const float4 v0, const float4 e1, const float4 e2,
+// The triangle predicate of hcc.h, operation by operation.  o = (ox, oy, oz, tmin), d = (dx, dy, dz, tmax).
+__device__ __forceinline__ bool tri_hit(const float4 o, const float4 d, const float4 v0, const float4 e1, const float4 e2,
                                         float &t, float &u, float &v) {
-    float px = fmaf(r.dy, e2.z, -(r.dz * e2.y));
-    float py = fmaf(r.dz, e2.x, -(r.dx * e2.z));
-    float pz = fmaf(r.dx, e2.y, -(r.dy * e2.x));
+    float px = fmaf(d.y, e2.z, -(d.z * e2.y));
+    float py = fmaf(d.z, e2.x, -(d.x * e2.z));
+    float pz = fmaf(d.x, e2.y, -(d.y * e2.x));
     float det = fmaf(e1.x, px, fmaf(e1.y, py, e1.z * pz));
     if (det == 0.0f) return false;
     float inv = 1.0f / det;
-    float sx = r.ox - v0.x, sy = r.oy - v0.y, sz = r.oz - v0.z;
+    float sx = o.x - v0.x, sy = o.y - v0.y, sz = o.z - v0.z;
     u = fmaf(sx, px, fmaf(sy, py, sz * pz)) * inv;
     if (!(u >= 0.0f)) return false;
     float qx = fmaf(sy, e1.z, -(sz * e1.y));
     float qy = fmaf(sz, e1.x, -(sx * e1.z));
     float qz = fmaf(sx, e1.y, -(sy * e1.x));
-    v = fmaf(r.dx, qx, fmaf(r.dy, qy, r.dz * qz)) * inv;
+    v = fmaf(d.x, qx, fmaf(d.y, qy, d.z * qz)) * inv;
     if (!(v >= 0.0f) || !(u + v <= 1.0f)) return false;
     t = fmaf(e2.x, qx, fmaf(e2.y, qy, e2.z * qz)) * inv;
-    return t > r.tmin && t < r.tmax;
+    return t > o.w && t < d.w;
 }
 
 struct TraceScene {
-    const uint32_t *qrec;
+    const uint32_t *wrec;
     const float4 *ttri;
     uint32_t root_ref;
     float q_lo[3], q_scale[3];
 };
 
 // ctl[0] = next ray rank (zeroed on the launch stream before every launch).
-// STATS: the same traversal also counts the pair records fetched (32 bytes each) and the
+// STATS: the same traversal also counts the wide-node records fetched (64 bytes each) and the
 // triangle records fetched (64 bytes each): stats[0], stats[1]; stats[2] = rays, stats[3] =
-// deepest stack seen; stats[4] = distinct pair records summed over warp-level node steps (what
+// deepest stack seen; stats[4] = distinct node records summed over warp-level node steps (what
 // a coherent warp saves), stats[5] = warp-level node steps, stats[6] = lanes taking part in
-// them.  Used for the diagnostics only, never timed.
+// them, stats[7] = warp-level triangle rounds (stats[1] / stats[7] = lanes busy per round).
+// Used for the diagnostics only, never timed.
 template <bool ANY, bool STATS>
 __global__ void __launch_bounds__(TRACE_THREADS, ANY ? TRACE_BLOCKS_PER_SM_ANY : TRACE_BLOCKS_PER_SM)
 k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__restrict__ perm, uint32_t n,
         void *__restrict__ hits, uint32_t *ctl, unsigned long long *stats) {
     __shared__ uint32_t s_stack[SMEM_STACK][TRACE_THREADS];
+    __shared__ float4 s_ray[TRACE_THREADS][2];                          // (o, tmin), (d, tmax) of the lane's ray
+    __shared__ unsigned long long s_key[ANY ? 1 : TRACE_THREADS];       // closest: ord(t) << 32 | prim of the best hit
+    __shared__ float2 s_uv[ANY ? 1 : TRACE_THREADS];
+    __shared__ uint32_t s_occ[ANY ? TRACE_THREADS : 1];                 // any: occluded flag
+    __shared__ uint8_t s_item[TRACE_WARPS][256];                        // owner lane << 3 | triangle of its leaf
     uint32_t l_stack[STACK_SIZE - SMEM_STACK];
-    const uint32_t tid = threadIdx.x, lane = tid & 31u;
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, wbase = tid & ~31u;
     const uint32_t lanes_below = (1u << lane) - 1u;
-    unsigned long long n_pairs = 0, n_tris = 0, n_rays = 0, n_sect = 0, n_steps = 0, n_lanes = 0;
+    uint8_t *const items = s_item[tid >> 5];
+    unsigned long long n_nodes = 0, n_tris = 0, n_rays = 0, n_sect = 0, n_steps = 0, n_lanes = 0, n_rounds = 0;
     uint32_t max_sp = 0;
 
     uint32_t w_next = 0, w_end = 0;      // the warp's current chunk of ranks
     bool exhausted = false, have = false;
-    uint32_t cur = 0, rid = 0;           // cur: 0 = ray finished, else a record reference
+    uint32_t cur = 0, rid = 0;           // cur: 0 = ray finished, else a reference
     int sp = 0;
-    Ray r;
+    float tmin = 0.f;
     float ix = 0.f, iy = 0.f, iz = 0.f;                                 // slab planes: t = (32768 + cell) * i + c
     float cnx = 0.f, cny = 0.f, cnz = 0.f, cfx = 0.f, cfy = 0.f, cfz = 0.f;   // c of the near / far planes
     uint32_t snx = SEL_LO, sny = SEL_LO, snz = SEL_LO;                  // near-plane selectors
-    float best_t = 0.f, best_u = 0.f, best_v = 0.f;                     // culling limit / the hit
-    uint32_t best_prim = HCC_MISS_PRIM;
+    float best_t = 0.f;                                                 // culling limit
 
     auto push = [&](uint32_t v) {
         if (sp < SMEM_STACK) s_stack[sp][tid] = v; else l_stack[sp - SMEM_STACK] = v;
@@ -166,8 +184,11 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
                     const uint32_t j = w_next + rank;
                     rid = perm ? ld_stream(perm + j) : j;
                     const float4 a = ld_stream4(rays + 2 * (size_t)rid), b = ld_stream4(rays + 2 * (size_t)rid + 1);
-                    r.ox = a.x; r.oy = a.y; r.oz = a.z; r.tmin = a.w;
-                    r.dx = b.x; r.dy = b.y; r.dz = b.z; r.tmax = b.w;
+                    s_ray[tid][0] = a;
+                    s_ray[tid][1] = b;
+                    if (ANY) s_occ[tid] = 0u;
+                    else s_key[tid] = ((unsigned long long)ord_of(b.w) << 32) | 0xFFFFFFFFull;
+                    tmin = a.w;
                     // the ray in grid units: g(t) = go + t * (d * scale); a zero (or denormal)
                     // direction component becomes a huge finite reciprocal so that no inf - inf
                     // arises: the ray then just does not move along that axis
@@ -190,7 +211,7 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
                     cny = -fmaf(gy, iy, py * ay); cfy = -fmaf(gy, iy, -(py * ay));
                     cnz = -fmaf(gz, iz, pz * az); cfz = -fmaf(gz, iz, -(pz * az));
                     snx = ix >= 0.0f ? SEL_LO : SEL_HI; sny = iy >= 0.0f ? SEL_LO : SEL_HI; snz = iz >= 0.0f ? SEL_LO : SEL_HI;
-                    best_t = r.tmax; best_u = 0.f; best_v = 0.f; best_prim = HCC_MISS_PRIM;
+                    best_t = b.w;
                     sp = 0;
                     cur = sc.root_ref;
                     have = true;
@@ -202,11 +223,12 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
         }
         if (__ballot_sync(0xFFFFFFFFu, have) == 0u) break;
 
-        // ---- node phase: while at least half of the live lanes want a node step
+        // ---- node phase: while enough of the live lanes want a node step
         {
             uint32_t m = __ballot_sync(0xFFFFFFFFu, cur != 0u && !(cur & HCC_REF_LEAF));
             const uint32_t live = __popc(__ballot_sync(0xFFFFFFFFu, cur != 0u));
-            const uint32_t need = (live + 1u) / 2u;
+            const uint32_t need = (live + HCC_TRACE_NODE_DEN - 1u) / HCC_TRACE_NODE_DEN;
+            const float INF = __int_as_float(0x7f800000);
             while (m != 0u && (uint32_t)__popc(m) >= need) {
                 if (STATS) {
                     const bool walking = cur != 0u && !(cur & HCC_REF_LEAF);
@@ -215,92 +237,128 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
                     if (lane == 0) { ++n_steps; n_lanes += __popc(m); }
                 }
                 if (cur != 0u && !(cur & HCC_REF_LEAF)) {
-                    const Words8 q = ld256(sc.qrec + 8 * (size_t)(cur - 1u));
-                    if (STATS) ++n_pairs;
+                    const uint32_t *rec = sc.wrec + 16 * (size_t)(cur - 1u);
+                    const Words8 A = ld256(rec), B = ld256(rec + 8);
+                    if (STATS) ++n_nodes;
                     const uint32_t sfx = snx ^ SEL_FLIP, sfy = sny ^ SEL_FLIP, sfz = snz ^ SEL_FLIP;
-                    float tn0 = max3(fmaf(cell_plane(q.w[0], snx), ix, cnx), fmaf(cell_plane(q.w[1], sny), iy, cny), fmaf(cell_plane(q.w[2], snz), iz, cnz));
-                    float tf0 = min3(fmaf(cell_plane(q.w[0], sfx), ix, cfx), fmaf(cell_plane(q.w[1], sfy), iy, cfy), fmaf(cell_plane(q.w[2], sfz), iz, cfz));
-                    float tn1 = max3(fmaf(cell_plane(q.w[3], snx), ix, cnx), fmaf(cell_plane(q.w[4], sny), iy, cny), fmaf(cell_plane(q.w[5], snz), iz, cnz));
-                    float tf1 = min3(fmaf(cell_plane(q.w[3], sfx), ix, cfx), fmaf(cell_plane(q.w[4], sfy), iy, cfy), fmaf(cell_plane(q.w[5], sfz), iz, cfz));
-                    tn0 = fmaxf(tn0, r.tmin); tn1 = fmaxf(tn1, r.tmin);
-                    tf0 = fminf(tf0, best_t); tf1 = fminf(tf1, best_t);     // a box starting AT best_t is kept
-                    const bool h0 = tn0 <= tf0, h1 = tn1 <= tf1;
-                    const uint32_t ref0 = q.w[6], ref1 = q.w[7];
-                    if (h0 && h1) {
-                        const bool swap = tn1 < tn0;
-                        push(swap ? ref0 : ref1);
-                        cur = swap ? ref1 : ref0;
-                    } else if (h0) cur = ref0;
-                    else if (h1) cur = ref1;
-                    else cur = pop();
+                    // child c: x, y, z words; a missed child gets the distance +inf
+#define HCC_BOX(X, Y, Z, D)                                                                                                              \
+    {                                                                                                                                    \
+        float tn = max3(fmaf(cell_plane(X, snx), ix, cnx), fmaf(cell_plane(Y, sny), iy, cny), fmaf(cell_plane(Z, snz), iz, cnz));         \
+        float tf = min3(fmaf(cell_plane(X, sfx), ix, cfx), fmaf(cell_plane(Y, sfy), iy, cfy), fmaf(cell_plane(Z, sfz), iz, cfz));         \
+        tn = fmaxf(tn, tmin);                                                                                                            \
+        tf = fminf(tf, best_t); /* a box starting AT best_t is kept */                                                                   \
+        D = tn <= tf ? tn : INF;                                                                                                         \
+    }
+                    float d0, d1, d2, d3;
+                    HCC_BOX(A.w[0], A.w[1], A.w[2], d0)
+                    HCC_BOX(A.w[3], A.w[4], A.w[5], d1)
+                    HCC_BOX(A.w[6], A.w[7], B.w[0], d2)
+                    HCC_BOX(B.w[1], B.w[2], B.w[3], d3)
+#undef HCC_BOX
+                    uint32_t r0 = B.w[4], r1 = B.w[5], r2 = B.w[6], r3 = B.w[7];
+                    {
+                        // tournament: (0,1) -> A, loser L1; (2,3) -> B, loser L2; (A,B) -> nearest, loser L3.
+                        // Pushed farthest-first by this partial order: the loser of the losing pair, the loser of
+                        // the winning pair, then L3.
+                        const bool s01 = d1 < d0, s23 = d3 < d2;
+                        const float dA = s01 ? d1 : d0, dL1 = s01 ? d0 : d1;
+                        const uint32_t rA = s01 ? r1 : r0, rL1 = s01 ? r0 : r1;
+                        const float dB = s23 ? d3 : d2, dL2 = s23 ? d2 : d3;
+                        const uint32_t rB = s23 ? r3 : r2, rL2 = s23 ? r2 : r3;
+                        const bool sAB = dB < dA;
+                        const float dW = sAB ? dB : dA, dL3 = sAB ? dA : dB;
+                        const uint32_t rW = sAB ? rB : rA, rL3 = sAB ? rA : rB;
+                        const float dFar = sAB ? dL1 : dL2, dMid = sAB ? dL2 : dL1;     // pair losers: losing side first
+                        const uint32_t rFar = sAB ? rL1 : rL2, rMid = sAB ? rL2 : rL1;
+                        if (dW < INF) {
+                            if (dFar < INF) push(rFar);
+                            if (dMid < INF) push(rMid);
+                            if (dL3 < INF) push(rL3);
+                            cur = rW;
+                        } else cur = pop();
+                    }
                 }
                 m = __ballot_sync(0xFFFFFFFFu, cur != 0u && !(cur & HCC_REF_LEAF));
             }
         }
-        // ---- triangle phase
-        if (ANY || HCC_TRACE_CLOSEST_STEPWISE) {
-            // one triangle per lane per iteration, while a quarter of the live lanes hold a leaf
-            uint32_t m = __ballot_sync(0xFFFFFFFFu, (cur & HCC_REF_LEAF) != 0u);
-            const uint32_t live = __popc(__ballot_sync(0xFFFFFFFFu, cur != 0u));
-            const uint32_t need = (live + HCC_TRACE_TRI_DEN - 1u) / HCC_TRACE_TRI_DEN;
-            while (m != 0u && (uint32_t)__popc(m) >= need) {
-                if (cur & HCC_REF_LEAF) {
-                    const uint32_t first = cur & 0x0FFFFFFFu, rem = (cur >> 28) & 7u;
-                    const Words8 A = ld256(reinterpret_cast<const uint32_t *>(sc.ttri + 4 * (size_t)first));
-                    const float4 e2 = __ldg(sc.ttri + 4 * (size_t)first + 2);
-                    if (STATS) ++n_tris;
-                    const float4 v0 = make_float4(__uint_as_float(A.w[0]), __uint_as_float(A.w[1]), __uint_as_float(A.w[2]), 0.f);
-                    const float4 e1 = make_float4(__uint_as_float(A.w[4]), __uint_as_float(A.w[5]), __uint_as_float(A.w[6]), 0.f);
-                    float t, u, v;
-                    const bool hit = tri_hit(r, v0, e1, e2, t, u, v);
+        // ---- triangle phase: the leaves held by the lanes become (owner, triangle) items, 32 tested per round
+        {
+            const bool leaf = (cur & HCC_REF_LEAF) != 0u;
+            const uint32_t cnt = leaf ? ((cur >> 28) & 7u) + 1u : 0u;
+            const uint32_t b0 = __ballot_sync(0xFFFFFFFFu, cnt & 1u), b1 = __ballot_sync(0xFFFFFFFFu, cnt & 2u),
+                           b2 = __ballot_sync(0xFFFFFFFFu, cnt & 4u), b3 = __ballot_sync(0xFFFFFFFFu, cnt & 8u);
+            const uint32_t total = __popc(b0) + 2u * __popc(b1) + 4u * __popc(b2) + 8u * __popc(b3);
+            if (total != 0u) {
+                const uint32_t pre = __popc(b0 & lanes_below) + 2u * __popc(b1 & lanes_below) + 4u * __popc(b2 & lanes_below) +
+                                     8u * __popc(b3 & lanes_below);
+                for (uint32_t k = 0; k < cnt; ++k) items[pre + k] = (uint8_t)((lane << 3) | k);
+                __syncwarp();
+                for (uint32_t base = 0; base < total; base += 32u) {
+                    const uint32_t j = base + lane;
+                    const bool active = j < total;
+                    const uint32_t it = active ? items[j] : 0u;
+                    const uint32_t owner = it >> 3;
+                    const uint32_t oref = __shfl_sync(0xFFFFFFFFu, cur, owner);
+                    bool hit = false;
+                    float t = 0.f, u = 0.f, v = 0.f;
+                    uint32_t prim = 0u;
+                    if (active) {
+                        const float4 *tp = sc.ttri + 4 * (size_t)((oref & 0x0FFFFFFFu) + (it & 7u));
+                        const Words8 T = ld256(reinterpret_cast<const uint32_t *>(tp));
+                        const float4 e2 = __ldg(tp + 2);
+                        const float4 ro = s_ray[wbase + owner][0], rd = s_ray[wbase + owner][1];
+                        const float4 v0 = make_float4(__uint_as_float(T.w[0]), __uint_as_float(T.w[1]), __uint_as_float(T.w[2]), 0.f);
+                        const float4 e1 = make_float4(__uint_as_float(T.w[4]), __uint_as_float(T.w[5]), __uint_as_float(T.w[6]), 0.f);
+                        prim = T.w[3];
+                        hit = tri_hit(ro, rd, v0, e1, e2, t, u, v);
+                        if (STATS) ++n_tris;
+                    }
+                    if (STATS && lane == 0) ++n_rounds;
                     if (ANY) {
-                        if (hit) { best_prim = 0u; sp = 0; cur = 0u; }
-                        else cur = rem == 0u ? pop() : (HCC_REF_LEAF | ((rem - 1u) << 28) | (first + 1u));
-                    } else {
-                        const uint32_t prim = A.w[3];
-                        if (hit && (t < best_t || (t == best_t && prim < best_prim))) { best_t = t; best_u = u; best_v = v; best_prim = prim; }
-                        cur = rem == 0u ? pop() : (HCC_REF_LEAF | ((rem - 1u) << 28) | (first + 1u));
+                        if (hit) s_occ[wbase + owner] = 1u;
+                    } else if (__ballot_sync(0xFFFFFFFFu, hit) != 0u) {
+                        const unsigned long long key = ((unsigned long long)ord_of(t) << 32) | prim;
+                        if (hit) atomicMin(&s_key[wbase + owner], key);
+                        __syncwarp();
+                        if (hit && s_key[wbase + owner] == key) s_uv[wbase + owner] = make_float2(u, v);
                     }
                 }
-                m = __ballot_sync(0xFFFFFFFFu, (cur & HCC_REF_LEAF) != 0u);
-            }
-        } else if (cur & HCC_REF_LEAF) {
-            const uint32_t first = cur & 0x0FFFFFFFu, cnt = ((cur >> 28) & 7u) + 1u;
-            for (uint32_t k = 0; k < cnt; ++k) {
-                const float4 *tp = sc.ttri + 4 * (size_t)(first + k);
-                const Words8 A = ld256(reinterpret_cast<const uint32_t *>(tp));
-                const float4 e2 = __ldg(tp + 2);
-                if (STATS) ++n_tris;
-                const float4 v0 = make_float4(__uint_as_float(A.w[0]), __uint_as_float(A.w[1]), __uint_as_float(A.w[2]), 0.f);
-                const float4 e1 = make_float4(__uint_as_float(A.w[4]), __uint_as_float(A.w[5]), __uint_as_float(A.w[6]), 0.f);
-                float t, u, v;
-                if (tri_hit(r, v0, e1, e2, t, u, v)) {
-                    const uint32_t prim = A.w[3];
-                    if (t < best_t || (t == best_t && prim < best_prim)) { best_t = t; best_u = u; best_v = v; best_prim = prim; }
+                __syncwarp();
+                if (leaf) {
+                    if (ANY) {
+                        if (s_occ[tid]) { sp = 0; cur = 0u; }
+                        else cur = pop();
+                    } else {
+                        best_t = float_of((uint32_t)(s_key[tid] >> 32));
+                        cur = pop();
+                    }
                 }
             }
-            cur = pop();
         }
-        __syncwarp();
         // ---- retire finished rays
         if (have && cur == 0u) {
-            if (ANY) reinterpret_cast<uint8_t *>(hits)[rid] = best_prim != HCC_MISS_PRIM ? 1 : 0;
+            if (ANY) reinterpret_cast<uint8_t *>(hits)[rid] = s_occ[tid] ? 1 : 0;
             else {
-                const bool hit = best_prim != HCC_MISS_PRIM;
+                const unsigned long long key = s_key[tid];
+                const uint32_t prim = (uint32_t)key;
+                const bool hit = prim != HCC_MISS_PRIM;
+                const float2 uv = hit ? s_uv[tid] : make_float2(0.f, 0.f);
                 reinterpret_cast<float4 *>(hits)[rid] =
-                    make_float4(hit ? best_t : __int_as_float(0x7f800000), __uint_as_float(best_prim), best_u, best_v);
+                    make_float4(hit ? float_of((uint32_t)(key >> 32)) : __int_as_float(0x7f800000), __uint_as_float(prim), uv.x, uv.y);
             }
             have = false;
         }
     }
     if (STATS) {
-        atomicAdd(&stats[0], n_pairs);
+        atomicAdd(&stats[0], n_nodes);
         atomicAdd(&stats[1], n_tris);
         atomicAdd(&stats[2], n_rays);
         atomicMax(&stats[3], (unsigned long long)max_sp);
         atomicAdd(&stats[4], n_sect);
         atomicAdd(&stats[5], n_steps);
         atomicAdd(&stats[6], n_lanes);
+        atomicAdd(&stats[7], n_rounds);
     }
 }
 
@@ -323,7 +381,7 @@ static int32_t trace_impl(const char *who, const hcc_bvh *bvh, const float *rays
     const uint32_t want = (uint32_t)((n + TRACE_THREADS - 1) / TRACE_THREADS);
     const uint32_t blocks = want < cap ? want : cap;
     TraceScene sc;
-    sc.qrec = bvh->d_qrec; sc.ttri = bvh->d_ttri; sc.root_ref = bvh->root_ref;
+    sc.wrec = bvh->d_wrec; sc.ttri = bvh->d_ttri; sc.root_ref = bvh->root_ref;
     for (int a = 0; a < 3; ++a) { sc.q_lo[a] = bvh->q_lo[a]; sc.q_scale[a] = bvh->q_scale[a]; }
     // every launch takes the next counter slot of the ring and zeroes it on its own stream first, so
     // launches in flight on different streams never share a counter (up to HCC_TRACE_SLOTS of them)

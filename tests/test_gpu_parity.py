@@ -300,8 +300,8 @@ def test_trace_stats_and_anc(hcc, dev_cases):
     d = dev_cases["room_small"]
     b = d["case"].bvh
     st = hcc.trace_stats(d["bvh"], d["diffuse"], None, hcc.TRACE_CLOSEST)
-    assert st["rays"] == d["diffuse"].shape[0] and st["pairs"] > 0 and st["tris"] > 0
-    assert st["max_stack"] <= b.max_depth
+    assert st["rays"] == d["diffuse"].shape[0] and st["nodes"] > 0 and st["tris"] > 0
+    assert st["max_stack"] <= 3 * b.max_depth   # a 4-wide step pushes up to three references
     cut = hcc.select_cut(d["bvh"], hcc.density(d["bvh"]), 1024, 32)
     keys = hcc.encode(d["diffuse"], cut)
     k_host = hcc.keys_to_numpy(keys)
