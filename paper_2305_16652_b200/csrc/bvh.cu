@@ -32,7 +32,8 @@ void set_error(const char *fmt, ...) {
 //   w[3c .. 3c+2] = child c (0..3) x, y, z:  lo cell | hi cell << 16
 //   w[12 + c]     = reference of child c
 //   reference, internal child: (index of its wide node) + 1                       (bit 31 clear)
-//   reference, leaf child    : 0x80000000 | (count-1) << 28 | first triangle slot
+//   reference, leaf child    : 0x80000000 | (count-1) << 28 | first triangle slot, count <= 4 (a leaf of
+//                              5..8 triangles gets a wide node of its own: two such halves, same box)
 //   unused slot              : reference 0, box lo cell 32767 / hi cell 0 (never hit)
 // Cells are indices of a uniform grid over the root box, g = (x - q_lo) * q_scale + 2 in fp32
 // (a monotone map, so containment survives it), lo = floor(g) - 1, hi = ceil(g) + 1, clamped to
@@ -53,16 +54,16 @@ struct GridFrame { float lo[3], scale[3]; };
 
 constexpr uint32_t WIDE_NONE = 0xFFFFFFFFu;
 
-// wchild: 4 binary node ids per wide node (WIDE_NONE = unused slot); wide_of: wide node index of a
-// binary node that heads a wide node.
-__global__ void k_build_wrec(const hcc_node *__restrict__ nodes, const uint32_t *__restrict__ wchild,
-                             const uint32_t *__restrict__ wide_of, uint32_t n_wide, GridFrame f,
+// wbox: per wide node and slot, the binary node whose box the slot carries (WIDE_NONE = unused slot);
+// wref: the slot's reference, made on the host.
+__global__ void k_build_wrec(const hcc_node *__restrict__ nodes, const uint32_t *__restrict__ wbox,
+                             const uint32_t *__restrict__ wref, uint32_t n_wide, GridFrame f,
                              uint32_t *__restrict__ wrec) {
     uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n_wide) return;
     uint32_t w[16];
     for (uint32_t c = 0; c < 4; ++c) {
-        const uint32_t id = wchild[4 * (size_t)k + c];
+        const uint32_t id = wbox[4 * (size_t)k + c];
         if (id == WIDE_NONE) {
             w[3 * c] = w[3 * c + 1] = w[3 * c + 2] = 0x00007FFFu;
             w[12 + c] = 0u;
@@ -78,7 +79,7 @@ __global__ void k_build_wrec(const hcc_node *__restrict__ nodes, const uint32_t 
             if (!(gl == gl) || !(gh == gh)) { ql = 0; qh = 32767; }
             w[3 * c + a] = (uint32_t)ql | ((uint32_t)qh << 16);
         }
-        w[12 + c] = ch.count == 0 ? wide_of[id] + 1u : (HCC_REF_LEAF | ((ch.count - 1u) << 28) | ch.left_or_first);
+        w[12 + c] = wref[4 * (size_t)k + c];
     }
     uint4 *out = reinterpret_cast<uint4 *>(wrec + 16 * (size_t)k);
     for (int q = 0; q < 4; ++q) out[q] = make_uint4(w[4 * q], w[4 * q + 1], w[4 * q + 2], w[4 * q + 3]);
@@ -227,23 +228,41 @@ extern "C" int32_t hcc_bvh_create(const hcc_node *nodes, uint32_t n_nodes, const
     }
     b->n_internal = (uint32_t)internal_ids.size();
     b->trace_calls = new std::atomic<uint32_t>(0u);
-    b->root_ref = nodes[0].count == 0 ? 1u : (HCC_REF_LEAF | ((nodes[0].count - 1u) << 28) | nodes[0].left_or_first);
 
     // ---- collapse to a 4-wide tree (host, one pass): wide node ids are handed out family by family
     //      (the internal children of one wide node are neighbours) in depth-first order
-    std::vector<uint32_t> wide_of(n_nodes, WIDE_NONE), wchild;
+    std::vector<uint32_t> wbox, wref;
     {
         auto area = [&](uint32_t i) {
             const hcc_node &nd = nodes[i];
             const float dx = nd.hi[0] - nd.lo[0], dy = nd.hi[1] - nd.lo[1], dz = nd.hi[2] - nd.lo[2];
             return dx * dy + dy * dz + dz * dx;
         };
-        std::vector<uint32_t> todo;        // binary nodes heading a wide node whose children are not yet chosen
+        auto leaf_ref = [](uint32_t first, uint32_t count) { return HCC_REF_LEAF | ((count - 1u) << 28) | first; };
         uint32_t n_wide = 0;
-        if (nodes[0].count == 0) { wide_of[0] = n_wide++; todo.push_back(0u); }
-        wchild.reserve(4 * (size_t)(n_nodes / 3 + 2));
+        auto new_wide = [&]() {
+            wbox.resize(4 * (size_t)(n_wide + 1), WIDE_NONE);
+            wref.resize(4 * (size_t)(n_wide + 1), 0u);
+            return n_wide++;
+        };
+        // reference of binary node i as a child (or as the root); internal nodes are queued for expansion
+        std::vector<std::pair<uint32_t, uint32_t>> todo;        // (wide node, binary node heading it)
+        auto ref_of = [&](uint32_t i) -> uint32_t {
+            const hcc_node &nd = nodes[i];
+            if (nd.count == 0) return new_wide() + 1u;
+            if (nd.count <= 4u) return leaf_ref(nd.left_or_first, nd.count);
+            const uint32_t w = new_wide();          // a big leaf: two halves under its own box
+            wbox[4 * (size_t)w] = wbox[4 * (size_t)w + 1] = i;
+            wref[4 * (size_t)w] = leaf_ref(nd.left_or_first, 4u);
+            wref[4 * (size_t)w + 1] = leaf_ref(nd.left_or_first + 4u, nd.count - 4u);
+            return w + 1u;
+        };
+        wbox.reserve(4 * (size_t)(n_nodes / 3 + 2));
+        wref.reserve(4 * (size_t)(n_nodes / 3 + 2));
+        b->root_ref = ref_of(0u);
+        if (nodes[0].count == 0) todo.push_back({b->root_ref - 1u, 0u});
         while (!todo.empty()) {
-            const uint32_t head = todo.back();
+            const uint32_t wide = todo.back().first, head = todo.back().second;
             todo.pop_back();
             uint32_t c[4] = {nodes[head].left_or_first, nodes[head].left_or_first + 1u, WIDE_NONE, WIDE_NONE};
             uint32_t nc = 2;
@@ -260,20 +279,20 @@ extern "C" int32_t hcc_bvh_create(const hcc_node *nodes, uint32_t n_nodes, const
                 c[pick] = l;
                 c[nc++] = l + 1u;
             }
-            const size_t at = 4 * (size_t)wide_of[head];
-            if (wchild.size() < at + 4) wchild.resize(at + 4, WIDE_NONE);
-            for (uint32_t k = 0; k < 4; ++k) wchild[at + k] = c[k];
-            for (uint32_t k = 0; k < nc; ++k)
-                if (nodes[c[k]].count == 0) wide_of[c[k]] = n_wide++;
+            uint32_t refs[4];
+            for (uint32_t k = 0; k < nc; ++k) refs[k] = ref_of(c[k]);    // may grow wbox / wref
+            for (uint32_t k = 0; k < nc; ++k) {
+                wbox[4 * (size_t)wide + k] = c[k];
+                wref[4 * (size_t)wide + k] = refs[k];
+            }
             for (uint32_t k = nc; k-- > 0;)
-                if (nodes[c[k]].count == 0) todo.push_back(c[k]);
+                if (nodes[c[k]].count == 0) todo.push_back({refs[k] - 1u, c[k]});
         }
-        wchild.resize(4 * (size_t)n_wide, WIDE_NONE);
         b->n_wide = n_wide;
     }
 
     float *d_tris = nullptr;
-    uint32_t *d_prim = nullptr, *d_wide_of = nullptr, *d_wchild = nullptr;
+    uint32_t *d_prim = nullptr, *d_wbox = nullptr, *d_wref = nullptr;
     cudaError_t e = cudaSuccess;
     auto alloc = [&](void **p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
     alloc((void **)&b->d_nodes, sizeof(hcc_node) * (size_t)n_nodes);
@@ -284,28 +303,29 @@ extern "C" int32_t hcc_bvh_create(const hcc_node *nodes, uint32_t n_nodes, const
     alloc((void **)&b->d_wrec, 64 * ((size_t)b->n_wide + 1));
     alloc((void **)&b->d_trace_ctl, 2 * HCC_TRACE_SLOTS * sizeof(uint32_t));
     alloc((void **)&b->d_ttri, sizeof(float4) * 4 * (size_t)n_tris);
-    alloc((void **)&d_wide_of, sizeof(uint32_t) * (size_t)n_nodes);
-    alloc((void **)&d_wchild, sizeof(uint32_t) * (wchild.size() + 4));
+    alloc((void **)&d_wbox, sizeof(uint32_t) * (wbox.size() + 4));
+    alloc((void **)&d_wref, sizeof(uint32_t) * (wref.size() + 4));
     alloc((void **)&d_tris, sizeof(float) * 9 * (size_t)n_tris);
     alloc((void **)&d_prim, sizeof(uint32_t) * (size_t)n_tris);
     if (e != cudaSuccess) {
         set_error("hcc_bvh_create: cudaMalloc failed: %s", cudaGetErrorString(e));
-        cudaFree(d_tris); cudaFree(d_prim); cudaFree(d_wide_of); cudaFree(d_wchild);
+        cudaFree(d_tris); cudaFree(d_prim); cudaFree(d_wbox); cudaFree(d_wref);
         hcc_bvh_destroy(b);
         return e == cudaErrorMemoryAllocation ? HCC_ERR_OUT_OF_MEMORY : HCC_ERR_CUDA;
     }
     auto fail = [&](cudaError_t err, const char *what) {
         set_error("hcc_bvh_create: %s: %s", what, cudaGetErrorString(err));
-        cudaFree(d_tris); cudaFree(d_prim); cudaFree(d_wide_of); cudaFree(d_wchild);
+        cudaFree(d_tris); cudaFree(d_prim); cudaFree(d_wbox); cudaFree(d_wref);
         hcc_bvh_destroy(b);
         return (int32_t)HCC_ERR_CUDA;
     };
     if ((e = cudaMemcpyAsync(b->d_nodes, nodes, sizeof(hcc_node) * (size_t)n_nodes, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy nodes");
     if ((e = cudaMemcpyAsync(d_tris, tris, sizeof(float) * 9 * (size_t)n_tris, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy triangles");
     if ((e = cudaMemcpyAsync(d_prim, prim_idx, sizeof(uint32_t) * (size_t)n_tris, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy prim_idx");
-    if ((e = cudaMemcpyAsync(d_wide_of, wide_of.data(), sizeof(uint32_t) * (size_t)n_nodes, cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy wide ids");
-    if (!wchild.empty() &&
-        (e = cudaMemcpyAsync(d_wchild, wchild.data(), sizeof(uint32_t) * wchild.size(), cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy wide children");
+    if (!wbox.empty() &&
+        ((e = cudaMemcpyAsync(d_wbox, wbox.data(), sizeof(uint32_t) * wbox.size(), cudaMemcpyHostToDevice, s)) != cudaSuccess ||
+         (e = cudaMemcpyAsync(d_wref, wref.data(), sizeof(uint32_t) * wref.size(), cudaMemcpyHostToDevice, s)) != cudaSuccess))
+        return fail(e, "copy wide nodes");
     if (!internal_ids.empty() &&
         (e = cudaMemcpyAsync(b->d_internal, internal_ids.data(), sizeof(uint32_t) * internal_ids.size(), cudaMemcpyHostToDevice, s)) != cudaSuccess) return fail(e, "copy internal ids");
     if ((e = cudaMemsetAsync(b->d_flags, 0, sizeof(uint32_t) * (size_t)n_nodes, s)) != cudaSuccess) return fail(e, "memset");
@@ -313,15 +333,15 @@ extern "C" int32_t hcc_bvh_create(const hcc_node *nodes, uint32_t n_nodes, const
     const uint32_t T = 256;
     k_parents<<<(n_nodes + T - 1) / T, T, 0, s>>>(b->d_nodes, n_nodes, b->d_parent);
     if (b->n_wide)
-        k_build_wrec<<<(b->n_wide + T - 1) / T, T, 0, s>>>(b->d_nodes, d_wchild, d_wide_of, b->n_wide, frame, b->d_wrec);
+        k_build_wrec<<<(b->n_wide + T - 1) / T, T, 0, s>>>(b->d_nodes, d_wbox, d_wref, b->n_wide, frame, b->d_wrec);
     k_convert_tris<<<(n_tris + T - 1) / T, T, 0, s>>>(d_tris, d_prim, n_tris, b->d_ttri);
     k_subtree_leaves<<<(n_nodes + T - 1) / T, T, 0, s>>>(b->d_nodes, b->d_parent, b->d_flags, n_nodes, b->d_leaves);
     if ((e = cudaGetLastError()) != cudaSuccess) return fail(e, "conversion kernels");
     if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return fail(e, "synchronise");
     cudaFree(d_tris);
     cudaFree(d_prim);
-    cudaFree(d_wide_of);
-    cudaFree(d_wchild);
+    cudaFree(d_wbox);
+    cudaFree(d_wref);
     *out = b;
     return HCC_OK;
 }

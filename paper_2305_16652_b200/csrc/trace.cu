@@ -3,16 +3,19 @@
 //
 // Design: persistent warps pull 32-ray chunks of the (sorted) order from an
 // atomic counter and refill finished lanes from the same chunk, so the rays of a warp stay
-// neighbours in the sorted order.  The warp alternates between two phases:
-//  - node phase: every lane that holds an internal reference fetches ONE 64-byte record of the
+// neighbours in the sorted order.  Every iteration of a warp is
+//  - a node step: every lane that holds an internal reference fetches ONE 64-byte record of the
 //    4-wide tree (bvh.cu: four quantised child boxes + four references, two 256-bit loads), tests
-//    the four boxes, descends into the nearest hit child and pushes the others; it runs while at
-//    least half of the live lanes take part;
-//  - triangle phase: the leaves the lanes hold are flattened into (ray, triangle) items and the
-//    WHOLE warp tests 32 items per round, whoever owns the rays: the ray of an item is read from
-//    shared memory, a hit is committed to the owner's slot with a 64-bit shared-memory atomicMin
-//    on (t, prim) (closest hit) or a flag store (any hit).
-// The traversal stack lives in shared memory (conflict-free) and spills to local memory.
+//    the four boxes, descends into the nearest hit child and pushes the others;
+//  - leaves are not visited by the lane that reaches them: the lane appends (leaf, owner lane) to
+//    the warp's leaf queue in shared memory and goes on with its stack, so it never waits for a
+//    triangle test (its culling distance is refreshed when the queue is drained);
+//  - triangle rounds, whenever the queue holds eight leaves (or too few lanes can walk): the WHOLE
+//    warp tests eight leaves, four lanes per leaf, whoever owns the rays: the ray of a leaf is read
+//    from shared memory, a hit is committed to the owner's slot with a 64-bit shared-memory
+//    atomicMin on (t, prim) (closest hit) or a flag store (any hit).
+// A ray retires when its stack is empty and its queued leaves have been tested.  The traversal
+// stack lives in shared memory (conflict-free) and spills to local memory.
 // Compiled with -fmad=false; fmaf() appears exactly where hcc.h states it for the triangle
 // predicate, which alone defines the results.
 #include "common.cuh"
@@ -30,17 +33,48 @@ constexpr int TRACE_THREADS = 128;
 #define HCC_TRACE_REFILL_AT 8
 #endif
 #ifndef HCC_TRACE_SMEM_STACK
-#define HCC_TRACE_SMEM_STACK 12
+#define HCC_TRACE_SMEM_STACK 16
 #endif
-#ifndef HCC_TRACE_NODE_DEN            // node phase goes on while 1/NODE_DEN of the live lanes hold an internal reference
-#define HCC_TRACE_NODE_DEN 2
+#ifndef HCC_TRACE_WALK_MIN            // with fewer lanes able to take a node step the leaf queue is drained first
+#define HCC_TRACE_WALK_MIN 16
+#endif
+#ifndef HCC_TRACE_ANY_ORDERED         // any hit: 1 = nearest child first (as closest hit), 0 = first hit child in slot order
+#define HCC_TRACE_ANY_ORDERED 1
 #endif
 constexpr int TRACE_BLOCKS_PER_SM = HCC_TRACE_BLOCKS_PER_SM, TRACE_BLOCKS_PER_SM_ANY = HCC_TRACE_BLOCKS_PER_SM_ANY;
 constexpr int SMEM_STACK = HCC_TRACE_SMEM_STACK;   // entries per thread in shared memory
-constexpr int STACK_SIZE = 3 * 63 + 4;  // hcc_bvh_create admits depth <= 63; a 4-wide step pushes at most 3
+constexpr int STACK_SIZE = 3 * 64 + 4;  // hcc_bvh_create admits depth <= 63 (+1 for a split leaf); a 4-wide step pushes at most 3
 constexpr uint32_t CHUNK = 32;          // rays a warp takes from the counter at a time
 constexpr uint32_t REFILL_AT = HCC_TRACE_REFILL_AT;   // idle lanes that trigger a refill
 constexpr int TRACE_WARPS = TRACE_THREADS / 32;
+constexpr uint32_t QCAP = 64;           // leaf queue entries per warp (a power of two >= 32 + 32)
+constexpr uint32_t ROUND_LEAVES = 8;    // leaves per triangle round: four lanes each
+
+// Shared memory of a CTA, addressed with 32-bit shared-window addresses:
+//   lane slots : 48 bytes per thread: ray (o, tmin | d, t_best) at +0 / +16 (t_best starts as tmax and is
+//                lowered by committed hits), closest: key ord(t) << 32 | prim at +32 and (u, v) at +40;
+//                any: occluded flag at +32
+//   leaf queues: QCAP x 8 bytes per warp: (leaf reference, owner lane)
+//   stacks     : SMEM_STACK rows of 128 words (a lane's entries are 512 bytes apart: conflict-free)
+constexpr uint32_t SLOT_BYTES = 48;
+constexpr uint32_t OFF_SLOTS = 0, OFF_QUEUE = OFF_SLOTS + SLOT_BYTES * TRACE_THREADS,
+                   OFF_STACK = OFF_QUEUE + 8 * QCAP * TRACE_WARPS, SMEM_BYTES = OFF_STACK + 512 * SMEM_STACK;
+
+__device__ __forceinline__ uint32_t lds32(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
+__device__ __forceinline__ void sts32(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ uint2 lds64(uint32_t a) { uint2 v; asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a) : "memory"); return v; }
+__device__ __forceinline__ void sts64(uint32_t a, uint32_t x, uint32_t y) { asm volatile("st.shared.v2.u32 [%0], {%1,%2};" ::"r"(a), "r"(x), "r"(y) : "memory"); }
+__device__ __forceinline__ float4 lds128(uint32_t a) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts128(uint32_t a, float4 v) {
+    asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(a), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ void atom_min64(uint32_t a, unsigned long long v) {
+    asm volatile("red.shared.min.u64 [%0], %1;" ::"r"(a), "l"(v) : "memory");
+}
 
 __device__ __forceinline__ float max3(float a, float b, float c) {
     float d;
@@ -92,7 +126,8 @@ __device__ __forceinline__ float float_of(uint32_t k) {
     return __uint_as_float(k ^ (((k >> 31) - 1u) | 0x80000000u));
 }
 
-// The triangle predicate of hcc.h, operation by operation.  o = (ox, oy, oz, tmin), d = (dx, dy, dz, tmax).
+// The triangle predicate of hcc.h, operation by operation, with the upper end left to the caller:
+// true <=> det != 0, u >= 0, v >= 0, u + v <= 1, t > tmin.   o = (ox, oy, oz, tmin), d = (dx, dy, dz, -).
 __device__ __forceinline__ bool tri_hit(const float4 o, const float4 d, const float4 v0, const float4 e1, const float4 e2,
                                         float &t, float &u, float &v) {
     float px = fmaf(d.y, e2.z, -(d.z * e2.y));
@@ -110,7 +145,7 @@ __device__ __forceinline__ bool tri_hit(const float4 o, const float4 d, const fl
     v = fmaf(d.x, qx, fmaf(d.y, qy, d.z * qz)) * inv;
     if (!(v >= 0.0f) || !(u + v <= 1.0f)) return false;
     t = fmaf(e2.x, qx, fmaf(e2.y, qy, e2.z * qz)) * inv;
-    return t > o.w && t < d.w;
+    return t > o.w;
 }
 
 struct TraceScene {
@@ -131,38 +166,80 @@ template <bool ANY, bool STATS>
 __global__ void __launch_bounds__(TRACE_THREADS, ANY ? TRACE_BLOCKS_PER_SM_ANY : TRACE_BLOCKS_PER_SM)
 k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__restrict__ perm, uint32_t n,
         void *__restrict__ hits, uint32_t *ctl, unsigned long long *stats) {
-    __shared__ uint32_t s_stack[SMEM_STACK][TRACE_THREADS];
-    __shared__ float4 s_ray[TRACE_THREADS][2];                          // (o, tmin), (d, tmax) of the lane's ray
-    __shared__ unsigned long long s_key[ANY ? 1 : TRACE_THREADS];       // closest: ord(t) << 32 | prim of the best hit
-    __shared__ float2 s_uv[ANY ? 1 : TRACE_THREADS];
-    __shared__ uint32_t s_occ[ANY ? TRACE_THREADS : 1];                 // any: occluded flag
-    __shared__ uint8_t s_item[TRACE_WARPS][256];                        // owner lane << 3 | triangle of its leaf
+    __shared__ __align__(16) unsigned char smem[SMEM_BYTES];
     uint32_t l_stack[STACK_SIZE - SMEM_STACK];
-    const uint32_t tid = threadIdx.x, lane = tid & 31u, wbase = tid & ~31u;
+    const uint32_t tid = threadIdx.x, lane = tid & 31u;
     const uint32_t lanes_below = (1u << lane) - 1u;
-    uint8_t *const items = s_item[tid >> 5];
+    const uint32_t sa = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t sa_slot = sa + OFF_SLOTS + SLOT_BYTES * tid;                  // this lane's slot
+    const uint32_t sa_wslots = sa + OFF_SLOTS + SLOT_BYTES * (tid & ~31u);       // slot of lane 0 of the warp
+    const uint32_t sa_queue = sa + OFF_QUEUE + 8u * QCAP * (tid >> 5);
+    const uint32_t st_base = sa + OFF_STACK + 4u * tid, st_limit = st_base + 512u * SMEM_STACK;
     unsigned long long n_nodes = 0, n_tris = 0, n_rays = 0, n_sect = 0, n_steps = 0, n_lanes = 0, n_rounds = 0;
     uint32_t max_sp = 0;
 
     uint32_t w_next = 0, w_end = 0;      // the warp's current chunk of ranks
+    uint32_t q_head = 0, q_tail = 0;     // leaf queue positions (warp-uniform, monotonic)
     bool exhausted = false, have = false;
-    uint32_t cur = 0, rid = 0;           // cur: 0 = ray finished, else a reference
-    int sp = 0;
+    uint32_t cur = 0, rid = 0;           // cur: 0 = nothing left to walk, else a reference
+    uint32_t pend_end = 0;               // queue position behind the lane's last queued leaf
+    uint32_t sp = st_base;               // address of the next free stack entry (rows beyond st_limit live in l_stack)
     float tmin = 0.f;
     float ix = 0.f, iy = 0.f, iz = 0.f;                                 // slab planes: t = (32768 + cell) * i + c
     float cnx = 0.f, cny = 0.f, cnz = 0.f, cfx = 0.f, cfy = 0.f, cfz = 0.f;   // c of the near / far planes
     uint32_t snx = SEL_LO, sny = SEL_LO, snz = SEL_LO;                  // near-plane selectors
     float best_t = 0.f;                                                 // culling limit
+    const float INF = __int_as_float(0x7f800000);
 
-    auto push = [&](uint32_t v) {
-        if (sp < SMEM_STACK) s_stack[sp][tid] = v; else l_stack[sp - SMEM_STACK] = v;
-        ++sp;
-        if (STATS) max_sp = max(max_sp, (uint32_t)sp);
+    auto push = [&](uint32_t v) {      // general form (the node step has its own fast path)
+        if (sp < st_limit) sts32(sp, v); else l_stack[(sp - st_limit) >> 9] = v;
+        sp += 512u;
     };
     auto pop = [&]() -> uint32_t {
-        if (sp == 0) return 0u;
-        --sp;
-        return sp < SMEM_STACK ? s_stack[sp][tid] : l_stack[sp - SMEM_STACK];
+        if (sp == st_base) return 0u;
+        sp -= 512u;
+        return sp < st_limit ? lds32(sp) : l_stack[(sp - st_limit) >> 9];
+    };
+
+    // one triangle round: the eight leaves at the head of the queue, four lanes per leaf
+    auto tri_round = [&]() {
+        const uint32_t pos = q_head + (lane >> 2);
+        const bool valid = (int32_t)(q_tail - pos) > 0;
+        const uint2 e = lds64(sa_queue + 8u * (pos & (QCAP - 1u)));      // (leaf reference, owner lane); stale if !valid
+        const uint32_t k = lane & 3u;
+        const bool active = valid && k <= ((e.x >> 28) & 7u);
+        const uint32_t sa_own = sa_wslots + SLOT_BYTES * e.y;
+        bool hit = false;
+        float t = 0.f, u = 0.f, v = 0.f;
+        uint32_t prim = 0u;
+        if (active) {
+            const float4 *tp = sc.ttri + 4 * (size_t)((e.x & 0x0FFFFFFFu) + k);
+            const Words8 T = ld256(reinterpret_cast<const uint32_t *>(tp));
+            const float4 e2 = __ldg(tp + 2);
+            const float4 ro = lds128(sa_own), rd = lds128(sa_own + 16u);
+            const float4 v0 = make_float4(__uint_as_float(T.w[0]), __uint_as_float(T.w[1]), __uint_as_float(T.w[2]), 0.f);
+            const float4 e1 = make_float4(__uint_as_float(T.w[4]), __uint_as_float(T.w[5]), __uint_as_float(T.w[6]), 0.f);
+            prim = T.w[3];
+            // closest: rd.w is the best t so far (tmax at first): later hits lose anyway, equal ones go to the key
+            hit = tri_hit(ro, rd, v0, e1, e2, t, u, v) && (ANY ? t < rd.w : t <= rd.w);
+            if (STATS) ++n_tris;
+        }
+        if (ANY) {
+            if (hit) sts32(sa_own + 32u, 1u);
+        } else if (__any_sync(0xFFFFFFFFu, hit)) {
+            const unsigned long long key = ((unsigned long long)ord_of(t) << 32) | prim;
+            if (hit) atom_min64(sa_own + 32u, key);
+            __syncwarp();
+            if (hit) {
+                const uint2 now = lds64(sa_own + 32u);
+                if (now.x == prim && now.y == (uint32_t)(key >> 32)) {   // this lane's hit is the best: publish t, u, v
+                    sts32(sa_own + 28u, __float_as_uint(t));
+                    sts64(sa_own + 40u, __float_as_uint(u), __float_as_uint(v));
+                }
+            }
+        }
+        if (STATS && lane == 0) ++n_rounds;
+        q_head += min(ROUND_LEAVES, q_tail - q_head);
     };
 
     for (;;) {
@@ -184,10 +261,14 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
                     const uint32_t j = w_next + rank;
                     rid = perm ? ld_stream(perm + j) : j;
                     const float4 a = ld_stream4(rays + 2 * (size_t)rid), b = ld_stream4(rays + 2 * (size_t)rid + 1);
-                    s_ray[tid][0] = a;
-                    s_ray[tid][1] = b;
-                    if (ANY) s_occ[tid] = 0u;
-                    else s_key[tid] = ((unsigned long long)ord_of(b.w) << 32) | 0xFFFFFFFFull;
+                    sts128(sa_slot, a);
+                    sts128(sa_slot + 16u, b);
+                    if (ANY) sts32(sa_slot + 32u, 0u);
+                    else {
+                        // every t < tmax gives a smaller key, every t >= tmax a larger one; low word = "no hit yet"
+                        const unsigned long long k0 = ((unsigned long long)ord_of(b.w) << 32) - 1ull;
+                        sts64(sa_slot + 32u, (uint32_t)k0, (uint32_t)(k0 >> 32));
+                    }
                     tmin = a.w;
                     // the ray in grid units: g(t) = go + t * (d * scale); a zero (or denormal)
                     // direction component becomes a huge finite reciprocal so that no inf - inf
@@ -212,8 +293,9 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
                     cnz = -fmaf(gz, iz, pz * az); cfz = -fmaf(gz, iz, -(pz * az));
                     snx = ix >= 0.0f ? SEL_LO : SEL_HI; sny = iy >= 0.0f ? SEL_LO : SEL_HI; snz = iz >= 0.0f ? SEL_LO : SEL_HI;
                     best_t = b.w;
-                    sp = 0;
+                    sp = st_base;
                     cur = sc.root_ref;
+                    pend_end = q_head;
                     have = true;
                     if (STATS) ++n_rays;
                 }
@@ -223,25 +305,22 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
         }
         if (__ballot_sync(0xFFFFFFFFu, have) == 0u) break;
 
-        // ---- node phase: while enough of the live lanes want a node step
+        // ---- node step
         {
-            uint32_t m = __ballot_sync(0xFFFFFFFFu, cur != 0u && !(cur & HCC_REF_LEAF));
-            const uint32_t live = __popc(__ballot_sync(0xFFFFFFFFu, cur != 0u));
-            const uint32_t need = (live + HCC_TRACE_NODE_DEN - 1u) / HCC_TRACE_NODE_DEN;
-            const float INF = __int_as_float(0x7f800000);
-            while (m != 0u && (uint32_t)__popc(m) >= need) {
-                if (STATS) {
-                    const bool walking = cur != 0u && !(cur & HCC_REF_LEAF);
-                    const uint32_t peers = __match_any_sync(0xFFFFFFFFu, walking ? cur : (0x40000000u | lane));
-                    if (walking && (peers & lanes_below) == 0u) ++n_sect;
-                    if (lane == 0) { ++n_steps; n_lanes += __popc(m); }
-                }
-                if (cur != 0u && !(cur & HCC_REF_LEAF)) {
-                    const uint32_t *rec = sc.wrec + 16 * (size_t)(cur - 1u);
-                    const Words8 A = ld256(rec), B = ld256(rec + 8);
-                    if (STATS) ++n_nodes;
-                    const uint32_t sfx = snx ^ SEL_FLIP, sfy = sny ^ SEL_FLIP, sfz = snz ^ SEL_FLIP;
-                    // child c: x, y, z words; a missed child gets the distance +inf
+            const bool walking = cur != 0u && !(cur & HCC_REF_LEAF);
+            if (STATS) {
+                const uint32_t m = __ballot_sync(0xFFFFFFFFu, walking);
+                const uint32_t peers = __match_any_sync(0xFFFFFFFFu, walking ? cur : (0x40000000u | lane));
+                if (walking && (peers & lanes_below) == 0u) ++n_sect;
+                if (lane == 0 && m != 0u) { ++n_steps; n_lanes += __popc(m); }
+                max_sp = max(max_sp, (sp - st_base) >> 9);
+            }
+            if (walking) {
+                const uint32_t *rec = sc.wrec + 16 * (size_t)(cur - 1u);
+                const Words8 A = ld256(rec), B = ld256(rec + 8);
+                if (STATS) ++n_nodes;
+                const uint32_t sfx = snx ^ SEL_FLIP, sfy = sny ^ SEL_FLIP, sfz = snz ^ SEL_FLIP;
+                // child c: x, y, z words; a missed child gets the distance +inf
 #define HCC_BOX(X, Y, Z, D)                                                                                                              \
     {                                                                                                                                    \
         float tn = max3(fmaf(cell_plane(X, snx), ix, cnx), fmaf(cell_plane(Y, sny), iy, cny), fmaf(cell_plane(Z, snz), iz, cnz));         \
@@ -250,102 +329,91 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
         tf = fminf(tf, best_t); /* a box starting AT best_t is kept */                                                                   \
         D = tn <= tf ? tn : INF;                                                                                                         \
     }
-                    float d0, d1, d2, d3;
-                    HCC_BOX(A.w[0], A.w[1], A.w[2], d0)
-                    HCC_BOX(A.w[3], A.w[4], A.w[5], d1)
-                    HCC_BOX(A.w[6], A.w[7], B.w[0], d2)
-                    HCC_BOX(B.w[1], B.w[2], B.w[3], d3)
+                float d0, d1, d2, d3;
+                HCC_BOX(A.w[0], A.w[1], A.w[2], d0)
+                HCC_BOX(A.w[3], A.w[4], A.w[5], d1)
+                HCC_BOX(A.w[6], A.w[7], B.w[0], d2)
+                HCC_BOX(B.w[1], B.w[2], B.w[3], d3)
 #undef HCC_BOX
-                    uint32_t r0 = B.w[4], r1 = B.w[5], r2 = B.w[6], r3 = B.w[7];
-                    {
-                        // tournament: (0,1) -> A, loser L1; (2,3) -> B, loser L2; (A,B) -> nearest, loser L3.
-                        // Pushed farthest-first by this partial order: the loser of the losing pair, the loser of
-                        // the winning pair, then L3.
-                        const bool s01 = d1 < d0, s23 = d3 < d2;
-                        const float dA = s01 ? d1 : d0, dL1 = s01 ? d0 : d1;
-                        const uint32_t rA = s01 ? r1 : r0, rL1 = s01 ? r0 : r1;
-                        const float dB = s23 ? d3 : d2, dL2 = s23 ? d2 : d3;
-                        const uint32_t rB = s23 ? r3 : r2, rL2 = s23 ? r2 : r3;
-                        const bool sAB = dB < dA;
-                        const float dW = sAB ? dB : dA, dL3 = sAB ? dA : dB;
-                        const uint32_t rW = sAB ? rB : rA, rL3 = sAB ? rA : rB;
-                        const float dFar = sAB ? dL1 : dL2, dMid = sAB ? dL2 : dL1;     // pair losers: losing side first
-                        const uint32_t rFar = sAB ? rL1 : rL2, rMid = sAB ? rL2 : rL1;
-                        if (dW < INF) {
-                            if (dFar < INF) push(rFar);
-                            if (dMid < INF) push(rMid);
-                            if (dL3 < INF) push(rL3);
-                            cur = rW;
-                        } else cur = pop();
-                    }
+                const uint32_t r0 = B.w[4], r1 = B.w[5], r2 = B.w[6], r3 = B.w[7];
+                uint32_t rW, rP0, rP1, rP2;          // next reference; pushed first .. last
+                bool hW, hP0, hP1, hP2;
+                if (!ANY || HCC_TRACE_ANY_ORDERED) {
+                    // tournament: (0,1) -> A, loser L1; (2,3) -> B, loser L2; (A,B) -> nearest, loser L3.
+                    // Pushed farthest-first by this partial order: the loser of the losing pair, the loser of
+                    // the winning pair, then L3.
+                    const bool s01 = d1 < d0, s23 = d3 < d2;
+                    const float dA = s01 ? d1 : d0, dL1 = s01 ? d0 : d1;
+                    const uint32_t rA = s01 ? r1 : r0, rL1 = s01 ? r0 : r1;
+                    const float dB = s23 ? d3 : d2, dL2 = s23 ? d2 : d3;
+                    const uint32_t rB = s23 ? r3 : r2, rL2 = s23 ? r2 : r3;
+                    const bool sAB = dB < dA;
+                    hW = (sAB ? dB : dA) < INF; rW = sAB ? rB : rA;
+                    hP2 = (sAB ? dA : dB) < INF; rP2 = sAB ? rA : rB;
+                    hP0 = (sAB ? dL1 : dL2) < INF; rP0 = sAB ? rL1 : rL2;     // pair losers: losing side first
+                    hP1 = (sAB ? dL2 : dL1) < INF; rP1 = sAB ? rL2 : rL1;
+                } else {
+                    // slot order: the first hit child is next, the others are pushed
+                    const bool h0 = d0 < INF, h1 = d1 < INF, h2 = d2 < INF, h3 = d3 < INF;
+                    hW = h0 || h1 || h2 || h3;
+                    rW = h0 ? r0 : h1 ? r1 : h2 ? r2 : r3;
+                    hP2 = h0 && h1; rP2 = r1;
+                    hP1 = (h0 || h1) && h2; rP1 = r2;
+                    hP0 = (h0 || h1 || h2) && h3; rP0 = r3;
                 }
-                m = __ballot_sync(0xFFFFFFFFu, cur != 0u && !(cur & HCC_REF_LEAF));
-            }
-        }
-        // ---- triangle phase: the leaves held by the lanes become (owner, triangle) items, 32 tested per round
-        {
-            const bool leaf = (cur & HCC_REF_LEAF) != 0u;
-            const uint32_t cnt = leaf ? ((cur >> 28) & 7u) + 1u : 0u;
-            const uint32_t b0 = __ballot_sync(0xFFFFFFFFu, cnt & 1u), b1 = __ballot_sync(0xFFFFFFFFu, cnt & 2u),
-                           b2 = __ballot_sync(0xFFFFFFFFu, cnt & 4u), b3 = __ballot_sync(0xFFFFFFFFu, cnt & 8u);
-            const uint32_t total = __popc(b0) + 2u * __popc(b1) + 4u * __popc(b2) + 8u * __popc(b3);
-            if (total != 0u) {
-                const uint32_t pre = __popc(b0 & lanes_below) + 2u * __popc(b1 & lanes_below) + 4u * __popc(b2 & lanes_below) +
-                                     8u * __popc(b3 & lanes_below);
-                for (uint32_t k = 0; k < cnt; ++k) items[pre + k] = (uint8_t)((lane << 3) | k);
-                __syncwarp();
-                for (uint32_t base = 0; base < total; base += 32u) {
-                    const uint32_t j = base + lane;
-                    const bool active = j < total;
-                    const uint32_t it = active ? items[j] : 0u;
-                    const uint32_t owner = it >> 3;
-                    const uint32_t oref = __shfl_sync(0xFFFFFFFFu, cur, owner);
-                    bool hit = false;
-                    float t = 0.f, u = 0.f, v = 0.f;
-                    uint32_t prim = 0u;
-                    if (active) {
-                        const float4 *tp = sc.ttri + 4 * (size_t)((oref & 0x0FFFFFFFu) + (it & 7u));
-                        const Words8 T = ld256(reinterpret_cast<const uint32_t *>(tp));
-                        const float4 e2 = __ldg(tp + 2);
-                        const float4 ro = s_ray[wbase + owner][0], rd = s_ray[wbase + owner][1];
-                        const float4 v0 = make_float4(__uint_as_float(T.w[0]), __uint_as_float(T.w[1]), __uint_as_float(T.w[2]), 0.f);
-                        const float4 e1 = make_float4(__uint_as_float(T.w[4]), __uint_as_float(T.w[5]), __uint_as_float(T.w[6]), 0.f);
-                        prim = T.w[3];
-                        hit = tri_hit(ro, rd, v0, e1, e2, t, u, v);
-                        if (STATS) ++n_tris;
-                    }
-                    if (STATS && lane == 0) ++n_rounds;
-                    if (ANY) {
-                        if (hit) s_occ[wbase + owner] = 1u;
-                    } else if (__ballot_sync(0xFFFFFFFFu, hit) != 0u) {
-                        const unsigned long long key = ((unsigned long long)ord_of(t) << 32) | prim;
-                        if (hit) atomicMin(&s_key[wbase + owner], key);
-                        __syncwarp();
-                        if (hit && s_key[wbase + owner] == key) s_uv[wbase + owner] = make_float2(u, v);
-                    }
-                }
-                __syncwarp();
-                if (leaf) {
-                    if (ANY) {
-                        if (s_occ[tid]) { sp = 0; cur = 0u; }
-                        else cur = pop();
-                    } else {
-                        best_t = float_of((uint32_t)(s_key[tid] >> 32));
-                        cur = pop();
-                    }
+                if (sp + 3u * 512u <= st_limit) {
+                    // all in shared memory: store unconditionally, advance if the child was hit
+                    sts32(sp, rP0); sp += hP0 ? 512u : 0u;
+                    sts32(sp, rP1); sp += hP1 ? 512u : 0u;
+                    sts32(sp, rP2); sp += hP2 ? 512u : 0u;
+                    if (hW) cur = rW;
+                    else if (sp == st_base) cur = 0u;
+                    else { sp -= 512u; cur = lds32(sp); }
+                } else {
+                    if (hP0) push(rP0);
+                    if (hP1) push(rP1);
+                    if (hP2) push(rP2);
+                    cur = hW ? rW : pop();
                 }
             }
         }
-        // ---- retire finished rays
-        if (have && cur == 0u) {
-            if (ANY) reinterpret_cast<uint8_t *>(hits)[rid] = s_occ[tid] ? 1 : 0;
+        // ---- leaves go to the queue, their lanes on with the stack (twice: siblings are often leaves too)
+        uint32_t lm = __ballot_sync(0xFFFFFFFFu, (cur & HCC_REF_LEAF) != 0u);
+#pragma unroll 1
+        for (int pass = 0; pass < 2 && lm != 0u && q_tail - q_head <= QCAP - 32u; ++pass) {
+            if (cur & HCC_REF_LEAF) {
+                const uint32_t pos = q_tail + __popc(lm & lanes_below);
+                sts64(sa_queue + 8u * (pos & (QCAP - 1u)), cur, lane);
+                pend_end = pos + 1u;
+                cur = pop();
+            }
+            q_tail += __popc(lm);
+            lm = __ballot_sync(0xFFFFFFFFu, (cur & HCC_REF_LEAF) != 0u);
+        }
+        // ---- triangle rounds: whenever eight leaves wait, or all of them when too few lanes can walk
+        if (q_tail != q_head) {
+            const uint32_t walkers = __popc(__ballot_sync(0xFFFFFFFFu, cur != 0u && !(cur & HCC_REF_LEAF)));
+            const bool drain = walkers < HCC_TRACE_WALK_MIN;
+            if (drain || q_tail - q_head >= ROUND_LEAVES) {
+                __syncwarp();
+                do tri_round(); while (q_tail - q_head >= ROUND_LEAVES || (drain && q_tail != q_head));
+                __syncwarp();
+                if (have) {
+                    if (ANY) { if (lds32(sa_slot + 32u)) { sp = st_base; cur = 0u; } }
+                    else best_t = __uint_as_float(lds32(sa_slot + 28u));
+                }
+            }
+        }
+        // ---- retire rays with nothing left to walk and no leaf in the queue
+        if (have && cur == 0u && (int32_t)(q_head - pend_end) >= 0) {
+            if (ANY) reinterpret_cast<uint8_t *>(hits)[rid] = lds32(sa_slot + 32u) ? 1 : 0;
             else {
-                const unsigned long long key = s_key[tid];
-                const uint32_t prim = (uint32_t)key;
-                const bool hit = prim != HCC_MISS_PRIM;
-                const float2 uv = hit ? s_uv[tid] : make_float2(0.f, 0.f);
+                const uint2 key = lds64(sa_slot + 32u);           // (prim, ord(t))
+                const bool hit = key.x != HCC_MISS_PRIM;
+                const uint2 uv = lds64(sa_slot + 40u);
                 reinterpret_cast<float4 *>(hits)[rid] =
-                    make_float4(hit ? float_of((uint32_t)(key >> 32)) : __int_as_float(0x7f800000), __uint_as_float(prim), uv.x, uv.y);
+                    make_float4(hit ? float_of(key.y) : INF, __uint_as_float(key.x), hit ? __uint_as_float(uv.x) : 0.f,
+                                hit ? __uint_as_float(uv.y) : 0.f);
             }
             have = false;
         }
