@@ -41,7 +41,7 @@ UNIT = "Mrays/s"
 #  trace : lane-operations = 34 per sibling-pair record (12 cell->float conversions, 12 fma, 8 min/max,
 #          2 compares: both quantised child boxes, trace.cu) + 36 per triangle test (the formula in
 #          include/hcc.h); encode: 26 per exact fp32 slab test (6 sub, 6 mul, 12 min/max, compare, bit).
-OPS_BOX, OPS_PAIR, OPS_TRI = 26, 34, 36
+OPS_BOX, OPS_NODE, OPS_TRI = 26, 68, 36
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the two trace kernels on config 2, from the
 # ncu --set full capture summarised in profiles/r1b_ncu_full.md (a profiler number, config "room" only)
 NCU_TRAFFIC_ROOM = {"diffuse": 41.140480e6 + 0.928000e6, "shadow": 79.290880e6 + 5.325568e6}
@@ -363,7 +363,7 @@ def run_ours(args):
         perm = hcc.sort(keys, info["bits_used"])
         st = hcc.trace_stats(bvh, rays, perm, mode)
         st0 = hcc.trace_stats(bvh, rays, None, mode)
-        ops = (st["pairs"] * OPS_PAIR + st["tris"] * OPS_TRI)
+        ops = (st["nodes"] * OPS_NODE + st["tris"] * OPS_TRI)
         diag[name] = {"anc_hcc": hcc.anc(keys0, perm), "anc_nosort": hcc.anc(keys0, None),
                       "node_bytes_per_ray": st["node_bytes_per_ray"], "tri_bytes_per_ray": st["tri_bytes_per_ray"],
                       "node_bytes_per_ray_nosort": st0["node_bytes_per_ray"], "max_stack": st["max_stack"],

@@ -259,7 +259,16 @@ extern "C" int32_t hcc_bvh_create(const hcc_node *nodes, uint32_t n_nodes, const
         };
         wbox.reserve(4 * (size_t)(n_nodes / 3 + 2));
         wref.reserve(4 * (size_t)(n_nodes / 3 + 2));
-        b->root_ref = ref_of(0u);
+        // the root reference is always a wide node (trace.cu never holds a leaf reference as its current
+        // node): a root leaf of up to four triangles becomes the only child of a wide node of its own
+        if (nodes[0].count != 0 && nodes[0].count <= 4u) {
+            const uint32_t w = new_wide();
+            wbox[4 * (size_t)w] = 0u;
+            wref[4 * (size_t)w] = leaf_ref(nodes[0].left_or_first, nodes[0].count);
+            b->root_ref = w + 1u;
+        } else {
+            b->root_ref = ref_of(0u);
+        }
         if (nodes[0].count == 0) todo.push_back({b->root_ref - 1u, 0u});
         while (!todo.empty()) {
             const uint32_t wide = todo.back().first, head = todo.back().second;

@@ -3,18 +3,21 @@
 //
 // Design: persistent warps pull 32-ray chunks of the (sorted) order from an
 // atomic counter and refill finished lanes from the same chunk, so the rays of a warp stay
-// neighbours in the sorted order.  Every iteration of a warp is
-//  - a node step: every lane that holds an internal reference fetches ONE 64-byte record of the
-//    4-wide tree (bvh.cu: four quantised child boxes + four references, two 256-bit loads), tests
-//    the four boxes, descends into the nearest hit child and pushes the others;
-//  - leaves are not visited by the lane that reaches them: the lane appends (leaf, owner lane) to
-//    the warp's leaf queue in shared memory and goes on with its stack, so it never waits for a
-//    triangle test (its culling distance is refreshed when the queue is drained);
-//  - triangle rounds, whenever the queue holds eight leaves (or too few lanes can walk): the WHOLE
-//    warp tests eight leaves, four lanes per leaf, whoever owns the rays: the ray of a leaf is read
-//    from shared memory, a hit is committed to the owner's slot with a 64-bit shared-memory
-//    atomicMin on (t, prim) (closest hit) or a flag store (any hit).
-// A ray retires when its stack is empty and its queued leaves have been tested.  The traversal
+// neighbours in the sorted order.  A warp alternates between
+//  - node steps: every lane that holds a reference to a wide node fetches its 64-byte record
+//    (bvh.cu: four quantised child boxes + four references, two 256-bit loads) and tests the four
+//    boxes.  Hit LEAF children are not visited by the lane: it appends (leaf, owner lane) entries to
+//    the warp's leaf queue in shared memory (slots handed out by one shared-memory atomic add), so
+//    neither the traversal stack nor `cur` ever holds a leaf and a lane never waits for a triangle
+//    test.  Hit INTERNAL children are ordered by entry distance: the nearest is next, the others
+//    are pushed.  Node steps repeat with two warp votes per step until a round of leaves waits;
+//  - triangle rounds: the WHOLE warp tests the leaves at the head of the queue, TRI_LPL lanes per
+//    leaf, whoever owns the rays: the ray of a leaf is read from its owner's shared-memory slot, a
+//    hit is committed there with a 64-bit atomic min on (t, prim) (closest hit) or a flag store
+//    (any hit); the owners refresh their culling distance afterwards;
+//  - retire + refill, batched: only when REFILL_AT lanes are finished (or nothing else can run)
+//    are their hits written and new rays loaded.
+// A ray is finished when its stack is empty and its queued leaves have been tested.  The traversal
 // stack lives in shared memory (conflict-free) and spills to local memory.
 // Compiled with -fmad=false; fmaf() appears exactly where hcc.h states it for the triangle
 // predicate, which alone defines the results.
@@ -24,10 +27,10 @@ namespace hcc {
 
 constexpr int TRACE_THREADS = 128;
 #ifndef HCC_TRACE_BLOCKS_PER_SM       // closest hit: CTAs of 128 threads per SM
-#define HCC_TRACE_BLOCKS_PER_SM 8
+#define HCC_TRACE_BLOCKS_PER_SM 7
 #endif
 #ifndef HCC_TRACE_BLOCKS_PER_SM_ANY
-#define HCC_TRACE_BLOCKS_PER_SM_ANY 8
+#define HCC_TRACE_BLOCKS_PER_SM_ANY 7
 #endif
 #ifndef HCC_TRACE_REFILL_AT
 #define HCC_TRACE_REFILL_AT 8
@@ -36,29 +39,38 @@ constexpr int TRACE_THREADS = 128;
 #define HCC_TRACE_SMEM_STACK 16
 #endif
 #ifndef HCC_TRACE_WALK_MIN            // with fewer lanes able to take a node step the leaf queue is drained first
-#define HCC_TRACE_WALK_MIN 16
+#define HCC_TRACE_WALK_MIN 8
 #endif
 #ifndef HCC_TRACE_ANY_ORDERED         // any hit: 1 = nearest child first (as closest hit), 0 = first hit child in slot order
 #define HCC_TRACE_ANY_ORDERED 1
+#endif
+#ifndef HCC_TRACE_LPL                 // lanes per leaf in a triangle round (4, 2 or 1): a round tests 32 / LPL leaves
+#define HCC_TRACE_LPL 2
+#endif
+#ifndef HCC_TRACE_LPL_ANY
+#define HCC_TRACE_LPL_ANY 2
 #endif
 constexpr int TRACE_BLOCKS_PER_SM = HCC_TRACE_BLOCKS_PER_SM, TRACE_BLOCKS_PER_SM_ANY = HCC_TRACE_BLOCKS_PER_SM_ANY;
 constexpr int SMEM_STACK = HCC_TRACE_SMEM_STACK;   // entries per thread in shared memory
 constexpr int STACK_SIZE = 3 * 64 + 4;  // hcc_bvh_create admits depth <= 63 (+1 for a split leaf); a 4-wide step pushes at most 3
 constexpr uint32_t CHUNK = 32;          // rays a warp takes from the counter at a time
-constexpr uint32_t REFILL_AT = HCC_TRACE_REFILL_AT;   // idle lanes that trigger a refill
+constexpr uint32_t REFILL_AT = HCC_TRACE_REFILL_AT;   // finished lanes that trigger retirement + refill
 constexpr int TRACE_WARPS = TRACE_THREADS / 32;
-constexpr uint32_t QCAP = 64;           // leaf queue entries per warp (a power of two >= 32 + 32)
-constexpr uint32_t ROUND_LEAVES = 8;    // leaves per triangle round: four lanes each
+// leaf queue entries per warp, a power of two: a node step appends at most 4 x 32 entries and starts with
+// fewer than a round's worth (<= 32) waiting
+constexpr uint32_t QCAP = 256;
 
 // Shared memory of a CTA, addressed with 32-bit shared-window addresses:
 //   lane slots : 48 bytes per thread: ray (o, tmin | d, t_best) at +0 / +16 (t_best starts as tmax and is
 //                lowered by committed hits), closest: key ord(t) << 32 | prim at +32 and (u, v) at +40;
 //                any: occluded flag at +32
-//   leaf queues: QCAP x 8 bytes per warp: (leaf reference, owner lane)
+//   leaf queues: QCAP x 8 bytes per warp: (leaf reference, owner lane); queue tails: one word per warp
 //   stacks     : SMEM_STACK rows of 128 words (a lane's entries are 512 bytes apart: conflict-free)
 constexpr uint32_t SLOT_BYTES = 48;
 constexpr uint32_t OFF_SLOTS = 0, OFF_QUEUE = OFF_SLOTS + SLOT_BYTES * TRACE_THREADS,
-                   OFF_STACK = OFF_QUEUE + 8 * QCAP * TRACE_WARPS, SMEM_BYTES = OFF_STACK + 512 * SMEM_STACK;
+                   OFF_TAIL = OFF_QUEUE + 8 * QCAP * TRACE_WARPS, OFF_STACK = OFF_TAIL + 16,
+                   SMEM_BYTES = OFF_STACK + 512 * SMEM_STACK;
+static_assert(TRACE_WARPS <= 4, "queue tails: one word per warp in 16 bytes");
 
 __device__ __forceinline__ uint32_t lds32(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
 __device__ __forceinline__ void sts32(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
@@ -74,6 +86,12 @@ __device__ __forceinline__ void sts128(uint32_t a, float4 v) {
 }
 __device__ __forceinline__ void atom_min64(uint32_t a, unsigned long long v) {
     asm volatile("red.shared.min.u64 [%0], %1;" ::"r"(a), "l"(v) : "memory");
+}
+
+__device__ __forceinline__ uint32_t atom_add32(uint32_t a, uint32_t v) {
+    uint32_t old;
+    asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(a), "r"(v) : "memory");
+    return old;
 }
 
 __device__ __forceinline__ float max3(float a, float b, float c) {
@@ -166,6 +184,9 @@ template <bool ANY, bool STATS>
 __global__ void __launch_bounds__(TRACE_THREADS, ANY ? TRACE_BLOCKS_PER_SM_ANY : TRACE_BLOCKS_PER_SM)
 k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__restrict__ perm, uint32_t n,
         void *__restrict__ hits, uint32_t *ctl, unsigned long long *stats) {
+    constexpr uint32_t LPL = ANY ? HCC_TRACE_LPL_ANY : HCC_TRACE_LPL;     // lanes per leaf in a triangle round
+    constexpr uint32_t ROUND_LEAVES = 32u / LPL;
+    static_assert(LPL == 1 || LPL == 2 || LPL == 4, "lanes per leaf");
     __shared__ __align__(16) unsigned char smem[SMEM_BYTES];
     uint32_t l_stack[STACK_SIZE - SMEM_STACK];
     const uint32_t tid = threadIdx.x, lane = tid & 31u;
@@ -174,14 +195,15 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
     const uint32_t sa_slot = sa + OFF_SLOTS + SLOT_BYTES * tid;                  // this lane's slot
     const uint32_t sa_wslots = sa + OFF_SLOTS + SLOT_BYTES * (tid & ~31u);       // slot of lane 0 of the warp
     const uint32_t sa_queue = sa + OFF_QUEUE + 8u * QCAP * (tid >> 5);
+    const uint32_t sa_tail = sa + OFF_TAIL + 4u * (tid >> 5);
     const uint32_t st_base = sa + OFF_STACK + 4u * tid, st_limit = st_base + 512u * SMEM_STACK;
     unsigned long long n_nodes = 0, n_tris = 0, n_rays = 0, n_sect = 0, n_steps = 0, n_lanes = 0, n_rounds = 0;
     uint32_t max_sp = 0;
 
     uint32_t w_next = 0, w_end = 0;      // the warp's current chunk of ranks
-    uint32_t q_head = 0, q_tail = 0;     // leaf queue positions (warp-uniform, monotonic)
+    uint32_t q_head = 0, q_tail = 0;     // leaf queue positions (warp-uniform, monotonic); the tail's master copy is in shared memory
     bool exhausted = false, have = false;
-    uint32_t cur = 0, rid = 0;           // cur: 0 = nothing left to walk, else a reference
+    uint32_t cur = 0, rid = 0;           // cur: 0 = nothing left to walk, else the reference of a wide node
     uint32_t pend_end = 0;               // queue position behind the lane's last queued leaf
     uint32_t sp = st_base;               // address of the next free stack entry (rows beyond st_limit live in l_stack)
     float tmin = 0.f;
@@ -190,6 +212,13 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
     uint32_t snx = SEL_LO, sny = SEL_LO, snz = SEL_LO;                  // near-plane selectors
     float best_t = 0.f;                                                 // culling limit
     const float INF = __int_as_float(0x7f800000);
+
+    if (lane == 0) sts32(sa_tail, 0u);
+    __syncwarp();
+#ifdef HCC_TRACE_TIMELINE   // debug builds only: per-warp start / exhaustion / end times behind the eight counters
+    unsigned long long tl_t0 = 0, tl_ex = 0;
+    if (stats) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tl_t0));
+#endif
 
     auto push = [&](uint32_t v) {      // general form (the node step has its own fast path)
         if (sp < st_limit) sts32(sp, v); else l_stack[(sp - st_limit) >> 9] = v;
@@ -201,28 +230,40 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
         return sp < st_limit ? lds32(sp) : l_stack[(sp - st_limit) >> 9];
     };
 
-    // one triangle round: the eight leaves at the head of the queue, four lanes per leaf
+    // one triangle round: the ROUND_LEAVES leaves at the head of the queue, LPL lanes per leaf; lane k of a
+    // leaf tests its triangles k, k + LPL, ... and commits the best of them
     auto tri_round = [&]() {
-        const uint32_t pos = q_head + (lane >> 2);
+        const uint32_t pos = q_head + lane / LPL;
         const bool valid = (int32_t)(q_tail - pos) > 0;
         const uint2 e = lds64(sa_queue + 8u * (pos & (QCAP - 1u)));      // (leaf reference, owner lane); stale if !valid
-        const uint32_t k = lane & 3u;
-        const bool active = valid && k <= ((e.x >> 28) & 7u);
+        const uint32_t last = (e.x >> 28) & 7u;                          // triangles of the leaf - 1
         const uint32_t sa_own = sa_wslots + SLOT_BYTES * e.y;
         bool hit = false;
         float t = 0.f, u = 0.f, v = 0.f;
         uint32_t prim = 0u;
-        if (active) {
-            const float4 *tp = sc.ttri + 4 * (size_t)((e.x & 0x0FFFFFFFu) + k);
-            const Words8 T = ld256(reinterpret_cast<const uint32_t *>(tp));
-            const float4 e2 = __ldg(tp + 2);
+        uint32_t k = lane % LPL;
+        if (valid && k <= last) {
             const float4 ro = lds128(sa_own), rd = lds128(sa_own + 16u);
-            const float4 v0 = make_float4(__uint_as_float(T.w[0]), __uint_as_float(T.w[1]), __uint_as_float(T.w[2]), 0.f);
-            const float4 e1 = make_float4(__uint_as_float(T.w[4]), __uint_as_float(T.w[5]), __uint_as_float(T.w[6]), 0.f);
-            prim = T.w[3];
-            // closest: rd.w is the best t so far (tmax at first): later hits lose anyway, equal ones go to the key
-            hit = tri_hit(ro, rd, v0, e1, e2, t, u, v) && (ANY ? t < rd.w : t <= rd.w);
-            if (STATS) ++n_tris;
+            const float4 *tp = sc.ttri + 4 * (size_t)((e.x & 0x0FFFFFFFu) + k);
+#pragma unroll 1
+            for (;;) {
+                const Words8 T = ld256(reinterpret_cast<const uint32_t *>(tp));
+                const float4 e2 = __ldg(tp + 2);
+                const float4 v0 = make_float4(__uint_as_float(T.w[0]), __uint_as_float(T.w[1]), __uint_as_float(T.w[2]), 0.f);
+                const float4 e1 = make_float4(__uint_as_float(T.w[4]), __uint_as_float(T.w[5]), __uint_as_float(T.w[6]), 0.f);
+                float t1, u1, v1;
+                // closest: rd.w is the best t so far (tmax at first): later hits lose anyway, equal ones go to the key
+                if (tri_hit(ro, rd, v0, e1, e2, t1, u1, v1) && (ANY ? t1 < rd.w : t1 <= rd.w)) {
+                    // the lane's own triangles: nearest first, equal t to the lower prim id
+                    if (ANY || !hit || t1 < t || (t1 == t && T.w[3] < prim)) { t = t1; u = u1; v = v1; prim = T.w[3]; }
+                    hit = true;
+                }
+                if (STATS) ++n_tris;
+                if (LPL == 4) break;
+                k += LPL;
+                if (k > last || (ANY && hit)) break;
+                tp += 4 * LPL;
+            }
         }
         if (ANY) {
             if (hit) sts32(sa_own + 32u, 1u);
@@ -243,99 +284,137 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
     };
 
     for (;;) {
-        // ---- refill idle lanes with the next ranks of the warp's chunk
-        uint32_t idle = __ballot_sync(0xFFFFFFFFu, !have);
-        if (!exhausted && (idle == 0xFFFFFFFFu || (uint32_t)__popc(idle) >= REFILL_AT)) {
-            while (idle) {
-                if (w_next == w_end) {
-                    uint32_t base = 0;
-                    if (lane == 0) base = atomicAdd(&ctl[0], CHUNK);
-                    base = __shfl_sync(0xFFFFFFFFu, base, 0);
-                    if (base >= n) { exhausted = true; break; }
-                    w_next = base;
-                    w_end = min(base + CHUNK, n);
-                }
-                const uint32_t avail = w_end - w_next;
-                const uint32_t rank = __popc(idle & lanes_below);
-                if (!have && rank < avail) {
-                    const uint32_t j = w_next + rank;
-                    rid = perm ? ld_stream(perm + j) : j;
-                    const float4 a = ld_stream4(rays + 2 * (size_t)rid), b = ld_stream4(rays + 2 * (size_t)rid + 1);
-                    sts128(sa_slot, a);
-                    sts128(sa_slot + 16u, b);
-                    if (ANY) sts32(sa_slot + 32u, 0u);
+        // ---- retire finished rays and refill their lanes, in batches of REFILL_AT (or when nothing else can run)
+        {
+            const bool done = have && cur == 0u && (int32_t)(q_head - pend_end) >= 0;
+            const uint32_t free_m = __ballot_sync(0xFFFFFFFFu, done || !have);
+            if (free_m == 0xFFFFFFFFu || (uint32_t)__popc(free_m) >= REFILL_AT) {
+                if (done) {
+                    if (ANY) reinterpret_cast<uint8_t *>(hits)[rid] = lds32(sa_slot + 32u) ? 1 : 0;
                     else {
-                        // every t < tmax gives a smaller key, every t >= tmax a larger one; low word = "no hit yet"
-                        const unsigned long long k0 = ((unsigned long long)ord_of(b.w) << 32) - 1ull;
-                        sts64(sa_slot + 32u, (uint32_t)k0, (uint32_t)(k0 >> 32));
+                        const uint2 key = lds64(sa_slot + 32u);           // (prim, ord(t))
+                        const bool hit = key.x != HCC_MISS_PRIM;
+                        const uint2 uv = lds64(sa_slot + 40u);
+                        reinterpret_cast<float4 *>(hits)[rid] =
+                            make_float4(hit ? float_of(key.y) : INF, __uint_as_float(key.x), hit ? __uint_as_float(uv.x) : 0.f,
+                                        hit ? __uint_as_float(uv.y) : 0.f);
                     }
-                    tmin = a.w;
-                    // the ray in grid units: g(t) = go + t * (d * scale); a zero (or denormal)
-                    // direction component becomes a huge finite reciprocal so that no inf - inf
-                    // arises: the ray then just does not move along that axis
-                    const float BIG = 1.2676506e30f;   // 2^100
-                    const float gx = ((a.x - sc.q_lo[0]) * sc.q_scale[0] + HCC_GRID_OFFSET) + 32768.0f;
-                    const float gy = ((a.y - sc.q_lo[1]) * sc.q_scale[1] + HCC_GRID_OFFSET) + 32768.0f;
-                    const float gz = ((a.z - sc.q_lo[2]) * sc.q_scale[2] + HCC_GRID_OFFSET) + 32768.0f;
-                    ix = 1.0f / (b.x * sc.q_scale[0]); iy = 1.0f / (b.y * sc.q_scale[1]); iz = 1.0f / (b.z * sc.q_scale[2]);
-                    ix = ix == ix ? fminf(fmaxf(ix, -BIG), BIG) : BIG;
-                    iy = iy == iy ? fminf(fmaxf(iy, -BIG), BIG) : BIG;
-                    iz = iz == iz ? fminf(fmaxf(iz, -BIG), BIG) : BIG;
-                    // t(plane) = plane * i - g * i.  The rounding of g, of i and of this sum moves the
-                    // ray by about (|g| + 65536) * 2^-22 cells at the box, so near planes are tested
-                    // HCC_TRACE_PAD times (|g| + 65536) cells earlier and far planes that much later (an
-                    // origin inside the scene: 1/8 cell; a distant origin: in proportion to its distance).
-                    const float px = (fabsf(gx) + 65536.0f) * HCC_TRACE_PAD, py = (fabsf(gy) + 65536.0f) * HCC_TRACE_PAD,
-                                pz = (fabsf(gz) + 65536.0f) * HCC_TRACE_PAD;
-                    const float ax = fabsf(ix), ay = fabsf(iy), az = fabsf(iz);
-                    cnx = -fmaf(gx, ix, px * ax); cfx = -fmaf(gx, ix, -(px * ax));
-                    cny = -fmaf(gy, iy, py * ay); cfy = -fmaf(gy, iy, -(py * ay));
-                    cnz = -fmaf(gz, iz, pz * az); cfz = -fmaf(gz, iz, -(pz * az));
-                    snx = ix >= 0.0f ? SEL_LO : SEL_HI; sny = iy >= 0.0f ? SEL_LO : SEL_HI; snz = iz >= 0.0f ? SEL_LO : SEL_HI;
-                    best_t = b.w;
-                    sp = st_base;
-                    cur = sc.root_ref;
-                    pend_end = q_head;
-                    have = true;
-                    if (STATS) ++n_rays;
+                    have = false;
                 }
-                w_next += min((uint32_t)__popc(idle), avail);
-                idle = __ballot_sync(0xFFFFFFFFu, !have);
+                uint32_t idle = free_m;
+                while (!exhausted && idle) {
+                    if (w_next == w_end) {
+                        uint32_t base = 0;
+                        if (lane == 0) base = atomicAdd(&ctl[0], CHUNK);
+                        base = __shfl_sync(0xFFFFFFFFu, base, 0);
+                        if (base >= n) {
+                            exhausted = true;
+#ifdef HCC_TRACE_TIMELINE
+                            if (stats) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tl_ex));
+#endif
+                            break;
+                        }
+                        w_next = base;
+                        w_end = min(base + CHUNK, n);
+                    }
+                    const uint32_t avail = w_end - w_next;
+                    const uint32_t rank = __popc(idle & lanes_below);
+                    if (!have && rank < avail) {
+                        const uint32_t j = w_next + rank;
+                        rid = perm ? ld_stream(perm + j) : j;
+                        const float4 a = ld_stream4(rays + 2 * (size_t)rid), b = ld_stream4(rays + 2 * (size_t)rid + 1);
+                        sts128(sa_slot, a);
+                        sts128(sa_slot + 16u, b);
+                        if (ANY) sts32(sa_slot + 32u, 0u);
+                        else {
+                            // every t < tmax gives a smaller key, every t >= tmax a larger one; low word = "no hit yet"
+                            const unsigned long long k0 = ((unsigned long long)ord_of(b.w) << 32) - 1ull;
+                            sts64(sa_slot + 32u, (uint32_t)k0, (uint32_t)(k0 >> 32));
+                        }
+                        tmin = a.w;
+                        // the ray in grid units: g(t) = go + t * (d * scale); a zero (or denormal)
+                        // direction component becomes a huge finite reciprocal so that no inf - inf
+                        // arises: the ray then just does not move along that axis
+                        const float BIG = 1.2676506e30f;   // 2^100
+                        const float gx = ((a.x - sc.q_lo[0]) * sc.q_scale[0] + HCC_GRID_OFFSET) + 32768.0f;
+                        const float gy = ((a.y - sc.q_lo[1]) * sc.q_scale[1] + HCC_GRID_OFFSET) + 32768.0f;
+                        const float gz = ((a.z - sc.q_lo[2]) * sc.q_scale[2] + HCC_GRID_OFFSET) + 32768.0f;
+                        ix = 1.0f / (b.x * sc.q_scale[0]); iy = 1.0f / (b.y * sc.q_scale[1]); iz = 1.0f / (b.z * sc.q_scale[2]);
+                        ix = ix == ix ? fminf(fmaxf(ix, -BIG), BIG) : BIG;
+                        iy = iy == iy ? fminf(fmaxf(iy, -BIG), BIG) : BIG;
+                        iz = iz == iz ? fminf(fmaxf(iz, -BIG), BIG) : BIG;
+                        // t(plane) = plane * i - g * i.  The rounding of g, of i and of this sum moves the
+                        // ray by about (|g| + 65536) * 2^-22 cells at the box, so near planes are tested
+                        // HCC_TRACE_PAD times (|g| + 65536) cells earlier and far planes that much later (an
+                        // origin inside the scene: 1/8 cell; a distant origin: in proportion to its distance).
+                        const float px = (fabsf(gx) + 65536.0f) * HCC_TRACE_PAD, py = (fabsf(gy) + 65536.0f) * HCC_TRACE_PAD,
+                                    pz = (fabsf(gz) + 65536.0f) * HCC_TRACE_PAD;
+                        const float ax = fabsf(ix), ay = fabsf(iy), az = fabsf(iz);
+                        cnx = -fmaf(gx, ix, px * ax); cfx = -fmaf(gx, ix, -(px * ax));
+                        cny = -fmaf(gy, iy, py * ay); cfy = -fmaf(gy, iy, -(py * ay));
+                        cnz = -fmaf(gz, iz, pz * az); cfz = -fmaf(gz, iz, -(pz * az));
+                        snx = ix >= 0.0f ? SEL_LO : SEL_HI; sny = iy >= 0.0f ? SEL_LO : SEL_HI; snz = iz >= 0.0f ? SEL_LO : SEL_HI;
+                        best_t = b.w;
+                        sp = st_base;
+                        cur = sc.root_ref;           // always a wide node (hcc_bvh_create)
+                        pend_end = q_head;
+                        have = true;
+                        if (STATS) ++n_rays;
+                    }
+                    w_next += min((uint32_t)__popc(idle), avail);
+                    idle = __ballot_sync(0xFFFFFFFFu, !have);
+                }
+                if (__ballot_sync(0xFFFFFFFFu, have) == 0u) break;
             }
         }
-        if (__ballot_sync(0xFFFFFFFFu, have) == 0u) break;
 
-        // ---- node step
-        {
-            const bool walking = cur != 0u && !(cur & HCC_REF_LEAF);
+        // ---- node steps, until a round of leaves waits or too few lanes can walk
+        uint32_t wm = __ballot_sync(0xFFFFFFFFu, cur != 0u);
+        while (wm != 0u) {
             if (STATS) {
-                const uint32_t m = __ballot_sync(0xFFFFFFFFu, walking);
-                const uint32_t peers = __match_any_sync(0xFFFFFFFFu, walking ? cur : (0x40000000u | lane));
-                if (walking && (peers & lanes_below) == 0u) ++n_sect;
-                if (lane == 0 && m != 0u) { ++n_steps; n_lanes += __popc(m); }
+                const uint32_t peers = __match_any_sync(0xFFFFFFFFu, cur != 0u ? cur : (0x40000000u | lane));
+                if (cur != 0u && (peers & lanes_below) == 0u) ++n_sect;
+                if (lane == 0) { ++n_steps; n_lanes += __popc(wm); }
                 max_sp = max(max_sp, (sp - st_base) >> 9);
             }
-            if (walking) {
+            if (cur != 0u) {
                 const uint32_t *rec = sc.wrec + 16 * (size_t)(cur - 1u);
                 const Words8 A = ld256(rec), B = ld256(rec + 8);
                 if (STATS) ++n_nodes;
                 const uint32_t sfx = snx ^ SEL_FLIP, sfy = sny ^ SEL_FLIP, sfz = snz ^ SEL_FLIP;
-                // child c: x, y, z words; a missed child gets the distance +inf
-#define HCC_BOX(X, Y, Z, D)                                                                                                              \
+                // child c: x, y, z words -> entry distance and "the ray meets the box before best_t"
+#define HCC_BOX(X, Y, Z, D, H)                                                                                                           \
     {                                                                                                                                    \
         float tn = max3(fmaf(cell_plane(X, snx), ix, cnx), fmaf(cell_plane(Y, sny), iy, cny), fmaf(cell_plane(Z, snz), iz, cnz));         \
         float tf = min3(fmaf(cell_plane(X, sfx), ix, cfx), fmaf(cell_plane(Y, sfy), iy, cfy), fmaf(cell_plane(Z, sfz), iz, cfz));         \
-        tn = fmaxf(tn, tmin);                                                                                                            \
+        D = fmaxf(tn, tmin);                                                                                                             \
         tf = fminf(tf, best_t); /* a box starting AT best_t is kept */                                                                   \
-        D = tn <= tf ? tn : INF;                                                                                                         \
+        H = D <= tf;                                                                                                                     \
     }
                 float d0, d1, d2, d3;
-                HCC_BOX(A.w[0], A.w[1], A.w[2], d0)
-                HCC_BOX(A.w[3], A.w[4], A.w[5], d1)
-                HCC_BOX(A.w[6], A.w[7], B.w[0], d2)
-                HCC_BOX(B.w[1], B.w[2], B.w[3], d3)
+                bool h0, h1, h2, h3;
+                HCC_BOX(A.w[0], A.w[1], A.w[2], d0, h0)
+                HCC_BOX(A.w[3], A.w[4], A.w[5], d1, h1)
+                HCC_BOX(A.w[6], A.w[7], B.w[0], d2, h2)
+                HCC_BOX(B.w[1], B.w[2], B.w[3], d3, h3)
 #undef HCC_BOX
                 const uint32_t r0 = B.w[4], r1 = B.w[5], r2 = B.w[6], r3 = B.w[7];
+                // hit leaves go to the warp's queue (slots from one shared-memory atomic add), never to the stack
+                const bool l0 = h0 && (int32_t)r0 < 0, l1 = h1 && (int32_t)r1 < 0, l2 = h2 && (int32_t)r2 < 0, l3 = h3 && (int32_t)r3 < 0;
+                const uint32_t nl = (l0 ? 1u : 0u) + (l1 ? 1u : 0u) + (l2 ? 1u : 0u) + (l3 ? 1u : 0u);
+                if (nl != 0u) {
+                    uint32_t pos = atom_add32(sa_tail, nl);
+                    if (l0) { sts64(sa_queue + 8u * (pos & (QCAP - 1u)), r0, lane); ++pos; }
+                    if (l1) { sts64(sa_queue + 8u * (pos & (QCAP - 1u)), r1, lane); ++pos; }
+                    if (l2) { sts64(sa_queue + 8u * (pos & (QCAP - 1u)), r2, lane); ++pos; }
+                    if (l3) { sts64(sa_queue + 8u * (pos & (QCAP - 1u)), r3, lane); ++pos; }
+                    pend_end = pos;
+                }
+                // hit wide nodes: a missed child, a leaf and an unused slot (reference 0, never hit) get +inf
+                d0 = h0 && (int32_t)r0 > 0 ? d0 : INF;
+                d1 = h1 && (int32_t)r1 > 0 ? d1 : INF;
+                d2 = h2 && (int32_t)r2 > 0 ? d2 : INF;
+                d3 = h3 && (int32_t)r3 > 0 ? d3 : INF;
                 uint32_t rW, rP0, rP1, rP2;          // next reference; pushed first .. last
                 bool hW, hP0, hP1, hP2;
                 if (!ANY || HCC_TRACE_ANY_ORDERED) {
@@ -354,12 +433,12 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
                     hP1 = (sAB ? dL2 : dL1) < INF; rP1 = sAB ? rL2 : rL1;
                 } else {
                     // slot order: the first hit child is next, the others are pushed
-                    const bool h0 = d0 < INF, h1 = d1 < INF, h2 = d2 < INF, h3 = d3 < INF;
-                    hW = h0 || h1 || h2 || h3;
-                    rW = h0 ? r0 : h1 ? r1 : h2 ? r2 : r3;
-                    hP2 = h0 && h1; rP2 = r1;
-                    hP1 = (h0 || h1) && h2; rP1 = r2;
-                    hP0 = (h0 || h1 || h2) && h3; rP0 = r3;
+                    const bool i0 = d0 < INF, i1 = d1 < INF, i2 = d2 < INF, i3 = d3 < INF;
+                    hW = i0 || i1 || i2 || i3;
+                    rW = i0 ? r0 : i1 ? r1 : i2 ? r2 : r3;
+                    hP2 = i0 && i1; rP2 = r1;
+                    hP1 = (i0 || i1) && i2; rP1 = r2;
+                    hP0 = (i0 || i1 || i2) && i3; rP0 = r3;
                 }
                 if (sp + 3u * 512u <= st_limit) {
                     // all in shared memory: store unconditionally, advance if the child was hit
@@ -376,26 +455,16 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
                     cur = hW ? rW : pop();
                 }
             }
+            __syncwarp();
+            q_tail = lds32(sa_tail);
+            wm = __ballot_sync(0xFFFFFFFFu, cur != 0u);
+            if (q_tail - q_head >= ROUND_LEAVES || (uint32_t)__popc(wm) < HCC_TRACE_WALK_MIN) break;
         }
-        // ---- leaves go to the queue, their lanes on with the stack (twice: siblings are often leaves too)
-        uint32_t lm = __ballot_sync(0xFFFFFFFFu, (cur & HCC_REF_LEAF) != 0u);
-#pragma unroll 1
-        for (int pass = 0; pass < 2 && lm != 0u && q_tail - q_head <= QCAP - 32u; ++pass) {
-            if (cur & HCC_REF_LEAF) {
-                const uint32_t pos = q_tail + __popc(lm & lanes_below);
-                sts64(sa_queue + 8u * (pos & (QCAP - 1u)), cur, lane);
-                pend_end = pos + 1u;
-                cur = pop();
-            }
-            q_tail += __popc(lm);
-            lm = __ballot_sync(0xFFFFFFFFu, (cur & HCC_REF_LEAF) != 0u);
-        }
-        // ---- triangle rounds: whenever eight leaves wait, or all of them when too few lanes can walk
+
+        // ---- triangle rounds: whenever a round's worth of leaves waits, or all of them when too few lanes can walk
         if (q_tail != q_head) {
-            const uint32_t walkers = __popc(__ballot_sync(0xFFFFFFFFu, cur != 0u && !(cur & HCC_REF_LEAF)));
-            const bool drain = walkers < HCC_TRACE_WALK_MIN;
+            const bool drain = (uint32_t)__popc(wm) < HCC_TRACE_WALK_MIN;
             if (drain || q_tail - q_head >= ROUND_LEAVES) {
-                __syncwarp();
                 do tri_round(); while (q_tail - q_head >= ROUND_LEAVES || (drain && q_tail != q_head));
                 __syncwarp();
                 if (have) {
@@ -404,20 +473,15 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
                 }
             }
         }
-        // ---- retire rays with nothing left to walk and no leaf in the queue
-        if (have && cur == 0u && (int32_t)(q_head - pend_end) >= 0) {
-            if (ANY) reinterpret_cast<uint8_t *>(hits)[rid] = lds32(sa_slot + 32u) ? 1 : 0;
-            else {
-                const uint2 key = lds64(sa_slot + 32u);           // (prim, ord(t))
-                const bool hit = key.x != HCC_MISS_PRIM;
-                const uint2 uv = lds64(sa_slot + 40u);
-                reinterpret_cast<float4 *>(hits)[rid] =
-                    make_float4(hit ? float_of(key.y) : INF, __uint_as_float(key.x), hit ? __uint_as_float(uv.x) : 0.f,
-                                hit ? __uint_as_float(uv.y) : 0.f);
-            }
-            have = false;
-        }
     }
+#ifdef HCC_TRACE_TIMELINE
+    if (stats && lane == 0) {
+        unsigned long long tl_t1;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tl_t1));
+        const size_t w = (size_t)blockIdx.x * TRACE_WARPS + (tid >> 5);
+        stats[8 + 3 * w] = tl_t0; stats[9 + 3 * w] = tl_ex; stats[10 + 3 * w] = tl_t1;
+    }
+#endif
     if (STATS) {
         atomicAdd(&stats[0], n_nodes);
         atomicAdd(&stats[1], n_tris);
@@ -457,6 +521,12 @@ static int32_t trace_impl(const char *who, const hcc_bvh *bvh, const float *rays
     uint32_t *ctl = bvh->d_trace_ctl + 2u * (bvh->trace_calls->fetch_add(1u) % (uint32_t)HCC_TRACE_SLOTS);
     HCC_CUDA_TRY(cudaMemsetAsync(ctl, 0, 2 * sizeof(uint32_t), s));
     const float4 *rays = (const float4 *)rays_dev;
+#ifdef HCC_TRACE_TIMELINE
+    if (stats_dev) {
+        if (mode == HCC_TRACE_CLOSEST) k_trace<false, false><<<blocks, TRACE_THREADS, 0, s>>>(sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, stats_dev);
+        else                           k_trace<true, false><<<blocks, TRACE_THREADS, 0, s>>>(sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, stats_dev);
+    } else
+#endif
     if (stats_dev) {
         if (mode == HCC_TRACE_CLOSEST) k_trace<false, true><<<blocks, TRACE_THREADS, 0, s>>>(sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, stats_dev);
         else                           k_trace<true, true><<<blocks, TRACE_THREADS, 0, s>>>(sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, stats_dev);

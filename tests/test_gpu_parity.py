@@ -493,23 +493,31 @@ def test_trace_root_leaf_bvh(hcc):
 
 
 def test_trace_deep_chain_bvh_spills_the_stack(hcc):
-    """A degenerate chain (depth 40 > the 16 shared-memory stack entries) of nested boxes whose
-    far child is always hit too: the per-thread stack spills to local memory and comes back."""
+    """A degenerate comb (depth 40) of nested boxes: every chain node has a small INTERNAL sibling (two
+    one-triangle leaves) that is hit too and lies farther than the rest of the chain, so it is pushed at
+    every level (leaves never go to the stack): the per-thread stack outgrows its shared-memory rows,
+    spills to local memory and comes back."""
     import hcc_inputs
     depth = 40
-    tris, nodes = [], []
-    # node 2k = internal, children (2k+1 = leaf with one triangle, 2k+2 = next internal / last leaf)
-    for k in range(depth + 1):
-        z = 0.02 * (k + 1)
-        tris.append([[0.1, 0.1, z], [0.9, 0.1, z], [0.1, 0.9, z]])
+    zs = [0.02 * (k + 1) for k in range(depth + 1)]
+    tris = []
+    for k in range(depth):          # S_k: two triangles side by side in the plane z_k
+        tris.append([[0.1, 0.1, zs[k]], [0.5, 0.1, zs[k]], [0.1, 0.9, zs[k]]])
+        tris.append([[0.5, 0.1, zs[k]], [0.9, 0.1, zs[k]], [0.5, 0.9, zs[k]]])
+    tris.append([[0.1, 0.1, zs[depth]], [0.9, 0.1, zs[depth]], [0.1, 0.9, zs[depth]]])
+    # chain node I_k at 2k (children S_k at 2k+1 and I_{k+1} at 2k+2); the last chain node (2*depth) is a leaf;
+    # the two leaves of S_k follow at 2*depth + 1 + 2k
+    nodes = [None] * (2 * depth + 1 + 2 * depth)
     for k in range(depth):
-        nodes.append(((0.1, 0.1, 0.02 * (k + 1)), (0.9, 0.9, 0.02 * (depth + 1)), 2 * k + 1, 0))
-        nodes.append(((0.1, 0.1, 0.02 * (k + 1)), (0.9, 0.9, 0.02 * (k + 1)), k, 1))
-    nodes.append(((0.1, 0.1, 0.02 * (depth + 1)), (0.9, 0.9, 0.02 * (depth + 1)), depth, 1))
+        nodes[2 * k] = ((0.1, 0.1, zs[k]), (0.9, 0.9, zs[depth]), 2 * k + 1, 0)
+        nodes[2 * k + 1] = ((0.1, 0.1, zs[k]), (0.9, 0.9, zs[k]), 2 * depth + 1 + 2 * k, 0)
+        nodes[2 * depth + 1 + 2 * k] = ((0.1, 0.1, zs[k]), (0.5, 0.9, zs[k]), 2 * k, 1)
+        nodes[2 * depth + 2 + 2 * k] = ((0.5, 0.1, zs[k]), (0.9, 0.9, zs[k]), 2 * k + 1, 1)
+    nodes[2 * depth] = ((0.1, 0.1, zs[depth]), (0.9, 0.9, zs[depth]), 2 * depth, 1)
     b = hcc_inputs.make_bvh(nodes, np.array(tris, dtype=np.float32))
-    assert b.max_depth == depth
-    # rays travelling in -z from above meet the LAST triangle first: the near child is always the
-    # deeper internal node, so every leaf on the way down is pushed
+    assert b.max_depth == depth + 1
+    # rays travelling in -z from above meet the LAST plane first: the nearest child is always the rest of
+    # the chain, so the small internal siblings on the way down are all pushed
     rays = _rand_rays(2000 + 5, 0xDEE9, lo=0.0, hi=1.0)
     rays[:, 2] = 2.0
     rays[:, 4:7] = (0.0, 0.0, -1.0)
