@@ -38,14 +38,57 @@ UNIT = "Mrays/s"
 
 # Algorithmic work per ray, stated in DESIGN.md "Rooflines":
 #  encode: 32 B ray read + key write;  sort: one histogram read + per pass read+write of (key, id)
-#  trace : lane-operations = 34 per sibling-pair record (12 cell->float conversions, 12 fma, 8 min/max,
-#          2 compares: both quantised child boxes, trace.cu) + 36 per triangle test (the formula in
+#  trace : lane-operations = 68 per wide-node record fetched (four quantised child boxes: 24 cell->float
+#          conversions, 24 fma, 16 min/max, 4 compares, trace.cu) + 36 per triangle test (the formula in
 #          include/hcc.h); encode: 26 per exact fp32 slab test (6 sub, 6 mul, 12 min/max, compare, bit).
 OPS_BOX, OPS_NODE, OPS_TRI = 26, 68, 36
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the two trace kernels on config 2, from the
-# ncu --set full capture summarised in profiles/r1b_ncu_full.md (a profiler number, config "room" only)
-NCU_TRAFFIC_ROOM = {"diffuse": 41.140480e6 + 0.928000e6, "shadow": 79.290880e6 + 5.325568e6}
 SM_COUNT, LANES_PER_SM = 148, 128
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_trace_traffic.md")
+KERNEL_SOURCES = ("paper_2305_16652_b200/csrc/trace.cu", "paper_2305_16652_b200/csrc/bvh.cu",
+                  "paper_2305_16652_b200/csrc/common.cuh")
+
+
+def sort_bytes(key_b, passes):
+    """Bytes per pair the sort moves through HBM: (algorithmic per SURVEY.md 8(d), what the kernels really move).
+    Algorithmic: one histogram read + per pass a read and a write of (key, id).  Real: the first pass reads no ids
+    (it synthesises them) and the last pass writes no keys (sort.cu)."""
+    algo = key_b + passes * 2 * (key_b + 4)
+    if passes == 0:
+        return 0, 0
+    if passes == 1:
+        real = key_b + key_b + 4
+    else:
+        real = key_b + (2 * key_b + 4) + (passes - 2) * 2 * (key_b + 4) + (key_b + 8)
+    return algo, real
+
+
+def kernel_source_hash():
+    """sha256 over the traversal kernel's sources: profiles/r2_trace_traffic.md records the hash its ncu capture
+    was taken at, so a stale capture is never reported (the GPU box has no .git to ask for HEAD)."""
+    import hashlib
+    h = hashlib.sha256()
+    for rel in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, rel), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload, batch):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the trace kernel from the tracked ncu summary, or
+    None when the file is missing, holds no line for this workload/batch or was captured from other sources."""
+    try:
+        want = kernel_source_hash()
+        with open(TRAFFIC_FILE) as f:
+            for line in f:
+                t = line.split()
+                if len(t) >= 6 and t[0] == "traffic" and t[1] == workload and t[2] == batch:
+                    kv = dict(x.split("=", 1) for x in t[3:] if "=" in x)
+                    if kv.get("sources") != want:
+                        return None
+                    return float(kv["dram_read_bytes"]) + float(kv["dram_write_bytes"])
+    except Exception:
+        return None
+    return None
 
 
 def _peaks():
@@ -183,17 +226,24 @@ def run_reference(args):
     return 0
 
 
-def _config(args, w, n_d, n_s, l2):
+def _config(args, w, n_d, n_s, l2, workload=None, world=None):
     names = {"room": "config 2 'room' of BASELINE.json", "fig1": "config 3 'Figure-1-like' of BASELINE.json",
              "large": "config 5 'large' of BASELINE.json", "tiny": "config 1 'tiny' of BASELINE.json"}
-    return {"workload": names[args.workload],
+    g = args.gpus if world is None else world
+    return {"workload": names[workload or args.workload],
             "triangles": int(w.bvh.n_tris), "bvh_nodes": int(w.bvh.n_nodes), "K": int(w.K),
             "key_bits": int(w.key_bits), "diffuse_rays": int(n_d), "shadow_rays": int(n_s),
             "resolution": f"{w.width}x{w.height}x{w.spp}spp", "bounce": int(getattr(args, "bounce", 1)), "l2": l2,
-            "parallelism": f"rays sharded over {args.gpus} GPU(s), BVH and cut replicated, no collective"}
+            "parallelism": (f"{g} rank(s), one per GPU: every rank runs the whole path on its own batches (weak scaling); BVH and "
+                            f"cut replicated, no collective on the data path; strong_scaling = one batch cut into contiguous ray ranges")}
 
 
 # ------------------------------------------------------------------------------------------
+class Scene:
+    """One workload on the device: BVH, cut, the two ray batches of one bounce, scratch."""
+    pass
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -201,6 +251,7 @@ def run_ours(args):
     from paper_2305_16652_b200 import build as cuda_build
     cuda_build.build()
     import paper_2305_16652_b200 as hcc
+    from paper_2305_16652_b200 import shard
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -211,119 +262,175 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     hbm_gbs, sm_max_mhz, peak_kind = _peaks()
-
-    # ---- inputs (seeded; rank r draws its own sub-pixel samples of the same scene)
-    w = hcc_inputs.Workload(args.workload, rank=rank, res_scale=args.res_scale)
-    b = w.bvh
-    bvh = hcc.Bvh(b.nodes, b.tris, b.prim_idx)
-
-    def gpu_trace_closest(_bvh, rays):
-        h = hcc.trace(bvh, torch.from_numpy(rays).cuda(), None, hcc.TRACE_CLOSEST)
-        t, p, _, _ = hcc.hits_to_numpy(h)
-        return t, p
-    diffuse_h, shadow_h = w.first_bounce(gpu_trace_closest)
-    for b_i in range(2, args.bounce + 1):      # later bounces: trace the previous diffuse batch, spawn the next
-        t_prev, p_prev = gpu_trace_closest(None, diffuse_h)
-        diffuse_h, shadow_h, _ = w.bounce(b_i, diffuse_h, t_prev, p_prev)
-    n_d, n_s = diffuse_h.shape[0], shadow_h.shape[0]
-    n = n_d + n_s
-    diffuse = torch.from_numpy(diffuse_h).cuda()
-    shadow = torch.from_numpy(shadow_h).cuda()
-    batches = ((diffuse, hcc.TRACE_CLOSEST, "diffuse"), (shadow, hcc.TRACE_ANY, "shadow"))
-
-    # ---- pre-process (once per scene): density + cut
+    alu_peak = SM_COUNT * LANES_PER_SM * sm_max_mhz * 1e6 / 1e12     # T lane-op/s
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    had = hcc.density(bvh)
-    cut = hcc.select_cut(bvh, had, w.K, w.key_bits)
-    torch.cuda.synchronize()
-    e0, e1 = ev(), ev()
-    e0.record()
-    hcc.density(bvh, out=had)
-    hcc.select_cut(bvh, had, w.K, w.key_bits, cut=cut)
-    e1.record()
-    torch.cuda.synchronize()
-    cut_ms = e0.elapsed_time(e1)
-    info = cut.info()
-    container = info["container_bits"]
-    passes = (info["bits_used"] + 7) // 8
-
-    pipe = hcc.Pipeline(max(n_d, n_s), 64, host_staging=True)
-    hits_d = torch.empty((n_d, 4), dtype=torch.float32, device="cuda")
-    hits_s = torch.empty(n_s, dtype=torch.uint8, device="cuda")
-    hits = {"diffuse": hits_d, "shadow": hits_s}
     flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.int32, device="cuda")   # 256 MiB > 126 MB L2
 
-    def step(order):
-        for rays, mode, name in batches:
-            pipe.reorder_trace(bvh, cut, order, rays, mode, hits=hits[name], key_bits=w.key_bits)
+    def max_over_ranks(x):
+        if world == 1:
+            return float(x)
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
 
-    def timed(order, steps, warmup, per_stage=False):
+    # ---- one workload on the device (seeded; rank r draws its own sub-pixel samples of the same scene)
+    def load(name, res_scale=1.0, seed_rank=0):
+        sc = Scene()
+        sc.name = name
+        sc.w = hcc_inputs.Workload(name, rank=seed_rank, res_scale=res_scale)
+        b = sc.w.bvh
+        sc.bvh = hcc.Bvh(b.nodes, b.tris, b.prim_idx)
+
+        def gpu_trace_closest(_bvh, rays):
+            h = hcc.trace(sc.bvh, torch.from_numpy(rays).cuda(), None, hcc.TRACE_CLOSEST)
+            t, p, _, _ = hcc.hits_to_numpy(h)
+            return t, p
+        sc.trace_closest = gpu_trace_closest
+        sc.had = hcc.density(sc.bvh)
+        sc.cut = hcc.select_cut(sc.bvh, sc.had, sc.w.K, sc.w.key_bits)
+        torch.cuda.synchronize()
+        e0, e1 = ev(), ev()
+        e0.record()
+        hcc.density(sc.bvh, out=sc.had)
+        hcc.select_cut(sc.bvh, sc.had, sc.w.K, sc.w.key_bits, cut=sc.cut)
+        e1.record()
+        torch.cuda.synchronize()
+        sc.cut_ms = e0.elapsed_time(e1)
+        sc.info = sc.cut.info()
+        sc.bounce_no, sc.host = 0, None
+        return sc
+
+    def set_bounce(sc, bounce, shuffle=False):
+        """Put the diffuse + shadow batches of `bounce` on the device (later bounces: trace the previous diffuse
+        batch with the library's own tracer, spawn the next).  shuffle: the same rays in a seeded random order."""
+        if sc.host is None or bounce < sc.bounce_no:
+            sc.host, sc.bounce_no = sc.w.first_bounce(sc.trace_closest), 1
+        while sc.bounce_no < bounce:
+            t_prev, p_prev = sc.trace_closest(None, sc.host[0])
+            d, s_, _ = sc.w.bounce(sc.bounce_no + 1, sc.host[0], t_prev, p_prev)
+            sc.host, sc.bounce_no = (d, s_), sc.bounce_no + 1
+        d_h, s_h = sc.host
+        sc.n_d, sc.n_s = d_h.shape[0], s_h.shape[0]
+        sc.n = sc.n_d + sc.n_s
+        diffuse, shadow = torch.from_numpy(d_h).cuda(), torch.from_numpy(s_h).cuda()
+        if shuffle:
+            g = torch.Generator(device="cuda").manual_seed(0x5EED)
+            diffuse = diffuse[torch.randperm(sc.n_d, device="cuda", generator=g)].contiguous()
+            shadow = shadow[torch.randperm(sc.n_s, device="cuda", generator=g)].contiguous()
+        sc.batches = ((diffuse, hcc.TRACE_CLOSEST, "diffuse"), (shadow, hcc.TRACE_ANY, "shadow"))
+        if getattr(sc, "pipe", None) is None or sc.pipe.n_max < max(sc.n_d, sc.n_s):
+            sc.pipe = hcc.Pipeline(max(sc.n_d, sc.n_s), 64, host_staging=(sc.name == args.workload))
+        sc.hits = {"diffuse": torch.empty((sc.n_d, 4), dtype=torch.float32, device="cuda"),
+                   "shadow": torch.empty(sc.n_s, dtype=torch.uint8, device="cuda")}
+
+    def step(sc, order):
+        for rays, mode, name in sc.batches:
+            sc.pipe.reorder_trace(sc.bvh, sc.cut, order, rays, mode, hits=sc.hits[name], key_bits=sc.w.key_bits)
+
+    def timed(sc, order, steps, warmup, per_stage=False):
         for _ in range(warmup):
-            step(order)
+            step(sc, order)
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
         pairs = [(ev(), ev()) for _ in range(steps)]
-        stage = {nm: {"encode": 0.0, "sort": 0.0, "trace": 0.0} for _, _, nm in batches}
+        stage = {nm: {"encode": 0.0, "sort": 0.0, "trace": 0.0} for _, _, nm in sc.batches}
         t0 = time.time()
-        for s, e in pairs:
+        for s_, e_ in pairs:
             flush.zero_()                       # L2 flush, outside the event bracket
-            s.record()
+            s_.record()
             if per_stage:
-                for rays, mode, name in batches:
-                    pipe.reorder_trace(bvh, cut, order, rays, mode, hits=hits[name], key_bits=w.key_bits)
-                    ms = pipe.stage_ms()
+                for rays, mode, name in sc.batches:
+                    sc.pipe.reorder_trace(sc.bvh, sc.cut, order, rays, mode, hits=sc.hits[name], key_bits=sc.w.key_bits)
+                    ms = sc.pipe.stage_ms()
                     for k in stage[name]:
                         stage[name][k] += ms[k] / steps
             else:
-                step(order)
-            e.record()
+                step(sc, order)
+            e_.record()
         torch.cuda.synchronize()
         t1 = time.time()
         if world > 1:
             dist.barrier()
-        ms = sum(s.elapsed_time(e) for s, e in pairs)
-        if world > 1:
-            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = max_over_ranks(sum(s_.elapsed_time(e_) for s_, e_ in pairs))
         return ms / steps, stage, (t0, t1)
+
+    ORDERS = (("hcc", hcc.ORDER_HCC), ("twopoint", hcc.ORDER_TWOPOINT), ("nosort", hcc.ORDER_NOSORT))
+
+    def compare(sc, k):
+        """Stage split of the three orders on the scene's current batches, and HCC's speed-ups."""
+        orders = {}
+        for name, order in ORDERS:
+            ms, stage, _ = timed(sc, order, k, 3, per_stage=True)
+            o = {"ms_per_step": ms, "mrays_per_s_incl": sc.n / ms / 1e3}
+            for bn, nb in (("diffuse", sc.n_d), ("shadow", sc.n_s)):
+                st = stage[bn]
+                tot = st["encode"] + st["sort"] + st["trace"]
+                o[bn] = {"encode_ms": st["encode"], "sort_ms": st["sort"], "trace_ms": st["trace"],
+                         "mrays_per_s_incl": nb / tot / 1e3, "mrays_per_s_trace_only": nb / st["trace"] / 1e3}
+            orders[name] = o
+        speed = {}
+        for bn in ("diffuse", "shadow"):
+            h = orders["hcc"][bn]
+            speed[bn] = {"incl_vs_nosort": h["mrays_per_s_incl"] / orders["nosort"][bn]["mrays_per_s_incl"],
+                         "incl_vs_twopoint": h["mrays_per_s_incl"] / orders["twopoint"][bn]["mrays_per_s_incl"],
+                         "trace_vs_nosort": h["mrays_per_s_trace_only"] / orders["nosort"][bn]["mrays_per_s_trace_only"],
+                         "trace_vs_twopoint": h["mrays_per_s_trace_only"] / orders["twopoint"][bn]["mrays_per_s_trace_only"]}
+        speed["all_incl_vs_nosort"] = orders["nosort"]["ms_per_step"] / orders["hcc"]["ms_per_step"]
+        speed["all_incl_vs_twopoint"] = orders["twopoint"]["ms_per_step"] / orders["hcc"]["ms_per_step"]
+        return orders, speed
+
+    def order_perms(sc, rays):
+        """The three traced orders of one batch as permutations (None = NoSort) and the HCC keys."""
+        keys = hcc.encode(rays, sc.cut)
+        keys0 = keys.clone()
+        perm = hcc.sort(keys, sc.info["bits_used"])
+        tk = hcc.encode_twopoint(rays, sc.bvh.scene_lo, sc.bvh.scene_hi, sc.w.key_bits)
+        perm_t = hcc.sort(tk, 6 * (sc.w.key_bits // 6))
+        return {"nosort": None, "twopoint": perm_t, "hcc": perm}, keys0
+
+    def counters(sc):
+        """What a warp shares: work counters of the instrumented traversal kernel (never timed) for the three orders
+        (coherent rays fetch the same nodes) and ANC."""
+        out = {}
+        for rays, mode, name in sc.batches:
+            perms, keys0 = order_perms(sc, rays)
+            o = {}
+            for on, pm in perms.items():
+                st = hcc.trace_stats(sc.bvh, rays, pm, mode)
+                o[on] = {"node_records_per_ray": st["nodes"] / max(st["rays"], 1), "tri_tests_per_ray": st["tris"] / max(st["rays"], 1),
+                         "distinct_records_per_warp_step": st["records_per_step"], "lanes_per_warp_step": st["lanes_per_step"],
+                         "lanes_per_tri_round": st["lanes_per_tri_round"], "max_stack": st["max_stack"],
+                         "lane_ops": st["nodes"] * OPS_NODE + st["tris"] * OPS_TRI}
+            out[name] = {"anc_hcc": hcc.anc(keys0, perms["hcc"]), "anc_nosort": hcc.anc(keys0, None), "orders": o}
+        return out
+
+    # =========================================================================== the headline workload
+    sc = load(args.workload, args.res_scale, seed_rank=rank)
+    set_bounce(sc, args.bounce)
+    w, bvh, cut, info = sc.w, sc.bvh, sc.cut, sc.info
+    n_d, n_s, n = sc.n_d, sc.n_s, sc.n
+    container = info["container_bits"]
+    passes = (info["bits_used"] + 7) // 8
+    pipe, hits_d, hits_s = sc.pipe, sc.hits["diffuse"], sc.hits["shadow"]
+    (diffuse, _, _), (shadow, _, _) = sc.batches
+    diffuse_h, shadow_h = sc.host
 
     # ---- the timed region: K steps of the HCC-ordered hot path
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
         time.sleep(0.3)
-    ms_step, _, (t0, t1) = timed(hcc.ORDER_HCC, args.steps, args.warmup)
+    ms_step, _, (t0, t1) = timed(sc, hcc.ORDER_HCC, args.steps, args.warmup)
     clocks = sampler.stop(t0, t1) if rank == 0 else None
     value = world * n / (ms_step * 1e-3) / 1e6
 
     # ---- stage split and the comparison orders on the same rays (short runs, same hygiene)
-    k_cmp = max(3, min(args.steps, 10))
-    orders = {}
-    for name, order in (("hcc", hcc.ORDER_HCC), ("twopoint", hcc.ORDER_TWOPOINT), ("nosort", hcc.ORDER_NOSORT)):
-        ms, stage, _ = timed(order, k_cmp, 3, per_stage=True)
-        o = {"ms_per_step": ms, "mrays_per_s_incl": n / ms / 1e3}
-        for bn, nb in (("diffuse", n_d), ("shadow", n_s)):
-            st = stage[bn]
-            tot = st["encode"] + st["sort"] + st["trace"]
-            o[bn] = {"encode_ms": st["encode"], "sort_ms": st["sort"], "trace_ms": st["trace"],
-                     "mrays_per_s_incl": nb / tot / 1e3, "mrays_per_s_trace_only": nb / st["trace"] / 1e3}
-        orders[name] = o
-    speed = {}
-    for bn in ("diffuse", "shadow"):
-        h = orders["hcc"][bn]
-        speed[bn] = {"incl_vs_nosort": h["mrays_per_s_incl"] / orders["nosort"][bn]["mrays_per_s_incl"],
-                     "incl_vs_twopoint": h["mrays_per_s_incl"] / orders["twopoint"][bn]["mrays_per_s_incl"],
-                     "trace_vs_nosort": h["mrays_per_s_trace_only"] / orders["nosort"][bn]["mrays_per_s_trace_only"],
-                     "trace_vs_twopoint": h["mrays_per_s_trace_only"] / orders["twopoint"][bn]["mrays_per_s_trace_only"]}
-    speed["all_incl_vs_nosort"] = orders["nosort"]["ms_per_step"] / orders["hcc"]["ms_per_step"]
-    speed["all_incl_vs_twopoint"] = orders["twopoint"]["ms_per_step"] / orders["hcc"]["ms_per_step"]
+    k_cmp = max(3, min(args.steps, 20))
+    orders, speed = compare(sc, k_cmp)
 
-    # ---- the same step with the two batches of the bounce on two streams (one pipeline each): the encode and
-    #      the latency-bound sort of one batch fill issue slots the other batch's traversal leaves idle.
-    #      Reported beside `value`, which stays the plain one-stream step.
+    # ---- the same step with the two batches of the bounce on two streams (one pipeline each)
     pipe2 = hcc.Pipeline(n_d, 64)
     streams_o = (torch.cuda.Stream(), torch.cuda.Stream())
 
@@ -331,7 +438,6 @@ def run_ours(args):
         cur = torch.cuda.current_stream()
         for st in streams_o:
             st.wait_stream(cur)
-        # shadow (the longer batch) first
         pipe.reorder_trace(bvh, cut, hcc.ORDER_HCC, shadow, hcc.TRACE_ANY, hits=hits_s, key_bits=w.key_bits, stream=streams_o[0])
         pipe2.reorder_trace(bvh, cut, hcc.ORDER_HCC, diffuse, hcc.TRACE_CLOSEST, hits=hits_d, key_bits=w.key_bits, stream=streams_o[1])
         for st in streams_o:
@@ -346,127 +452,197 @@ def run_ours(args):
         s0.record(); step_overlapped(); e0.record()
         torch.cuda.synchronize()
         ov.append(s0.elapsed_time(e0))
-    ov_ms = float(np.mean(ov))
-    if world > 1:
-        t = torch.tensor([ov_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ov_ms = float(t.item())
+    ov_ms = max_over_ranks(float(np.mean(ov)))
     overlapped = {"ms_per_step": ov_ms, "value": world * n / ov_ms / 1e3, "unit": UNIT,
                   "how": "diffuse and shadow batch of the step on two streams, one hcc_pipeline each"}
+    del pipe2
 
-    # ---- trace work counters (instrumented kernel, never timed) and ANC, HCC order
-    diag = {}
-    alu_peak = SM_COUNT * LANES_PER_SM * sm_max_mhz * 1e6 / 1e12     # T lane-op/s
-    for rays, mode, name in batches:
-        keys = hcc.encode(rays, cut)
-        keys0 = keys.clone()
-        perm = hcc.sort(keys, info["bits_used"])
-        st = hcc.trace_stats(bvh, rays, perm, mode)
-        st0 = hcc.trace_stats(bvh, rays, None, mode)
-        ops = (st["nodes"] * OPS_NODE + st["tris"] * OPS_TRI)
-        diag[name] = {"anc_hcc": hcc.anc(keys0, perm), "anc_nosort": hcc.anc(keys0, None),
-                      "node_bytes_per_ray": st["node_bytes_per_ray"], "tri_bytes_per_ray": st["tri_bytes_per_ray"],
-                      "node_bytes_per_ray_nosort": st0["node_bytes_per_ray"], "max_stack": st["max_stack"],
-                      "lane_ops_per_ray": ops / rays.shape[0], "lane_ops": ops}
+    # ---- strong scaling over the ranks: ONE batch pair (rank 0's samples) cut into contiguous ray ranges
+    #      (shard.ray_shard), every rank running hcc_reorder_trace on its range; no collective on the data path,
+    #      the hits are gathered once afterwards
+    strong = None
+    if world > 1:
+        sc0 = sc if rank == 0 else load(args.workload, args.res_scale, seed_rank=0)
+        if sc0 is not sc:
+            set_bounce(sc0, args.bounce)
+        spipe = hcc.Pipeline(max(shard.ray_shard(sc0.n_s, 0, world)[1], 1), 64)
+
+        def sstep():
+            return [shard.sharded_reorder_trace(spipe, sc0.bvh, sc0.cut, hcc.ORDER_HCC, rays, mode, rank, world,
+                                                key_bits=sc0.w.key_bits)[0] for rays, mode, _ in sc0.batches]
+        for _ in range(3):
+            sstep()
+        torch.cuda.synchronize()
+        dist.barrier()
+        tot = 0.0
+        for _ in range(k_cmp):
+            flush.zero_()
+            s0, e0 = ev(), ev()
+            s0.record(); loc = sstep(); e0.record()
+            torch.cuda.synchronize()
+            tot += s0.elapsed_time(e0) / k_cmp
+        dist.barrier()
+        s_ms = max_over_ranks(tot)
+        full_d = shard.gather_hits(loc[0], sc0.n_d)     # once, for the consumer; not part of the path
+        full_s = shard.gather_hits(loc[1], sc0.n_s)
+        ok = True
+        if rank == 0:
+            ok = bool(torch.equal(full_d.view(torch.int32), hcc.trace(sc0.bvh, sc0.batches[0][0], None, hcc.TRACE_CLOSEST).view(torch.int32))
+                      and torch.equal(full_s, hcc.trace(sc0.bvh, sc0.batches[1][0], None, hcc.TRACE_ANY)))
+        strong = {"ms_per_step": s_ms, "value": sc0.n / s_ms / 1e3, "unit": UNIT, "scaling": "strong", "ranks": world,
+                  "rays_total": sc0.n, "gathered_hits_equal_unsharded": ok,
+                  "how": "one bounce's batches cut into contiguous ray ranges by shard.ray_shard, one range per rank"}
+
+    # ---- trace work counters for the three orders (instrumented kernel, never timed) and ANC
+    diag = counters(sc)
     nrays = {"diffuse": n_d, "shadow": n_s}
     key_b = container // 8
+    sb_algo, sb_real = sort_bytes(key_b, passes)
     stages = {}
     for name in ("diffuse", "shadow"):
         o, nb = orders["hcc"][name], nrays[name]
-        enc_bytes = nb * (32 + key_b)
-        sort_bytes = nb * (key_b + passes * 2 * (key_b + 4))
-        enc_gbs = enc_bytes / (o["encode_ms"] * 1e-3) / 1e9
-        sort_gbs = sort_bytes / (o["sort_ms"] * 1e-3) / 1e9
-        tr = diag[name]["lane_ops"] / (o["trace_ms"] * 1e-3) / 1e12
+        enc_gbs = nb * (32 + key_b) / (o["encode_ms"] * 1e-3) / 1e9
+        sort_gbs = nb * sb_real / (o["sort_ms"] * 1e-3) / 1e9
+        tr = diag[name]["orders"]["hcc"]["lane_ops"] / (o["trace_ms"] * 1e-3) / 1e12
         enc_ops = nb * info["bits_used"] * OPS_BOX / (o["encode_ms"] * 1e-3) / 1e12
         stages[name] = {
             "encode": {"bound": "hbm", "achieved": enc_gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": enc_gbs / hbm_gbs,
                        "alu_achieved_tlaneops": enc_ops, "alu_frac": enc_ops / alu_peak, "box_tests_per_ray": info["bits_used"]},
             "sort": {"bound": "hbm", "achieved": sort_gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": sort_gbs / hbm_gbs,
-                     "passes": passes},
+                     "passes": passes, "bytes_per_pair_moved": sb_real, "bytes_per_pair_survey": sb_algo,
+                     "frac_survey_bytes": nb * sb_algo / (o["sort_ms"] * 1e-3) / 1e9 / hbm_gbs},
             "trace": {"bound": "alu", "achieved": tr, "peak": alu_peak, "unit": "Tlaneop/s", "frac": tr / alu_peak}}
-    # dominant kernel of the step = the closest-hit traversal of the diffuse batch
+    # dominant kernel of the step
     dom = max((("diffuse", "trace"), ("shadow", "trace"), ("diffuse", "sort"), ("shadow", "sort"),
                ("diffuse", "encode"), ("shadow", "encode")), key=lambda k: orders["hcc"][k[0]][k[1] + "_ms"])
     roof = dict(stages[dom[0]][dom[1]])
+    plain = dom[1] == "trace" and args.bounce == 1 and args.res_scale == 1.0 and world == 1
     roof = {"bound": roof["bound"], "achieved": roof["achieved"], "peak": roof["peak"], "unit": roof["unit"],
             "frac": roof["frac"],
-            "traffic": NCU_TRAFFIC_ROOM[dom[0]] if (args.workload == "room" and dom[1] == "trace" and args.bounce == 1 and args.res_scale == 1.0) else None,
-            "traffic_unit": "bytes per launch (dram read + write, ncu, profiles/r1b_ncu_full.md)",
+            "traffic": ncu_traffic(args.workload, dom[0]) if plain else None,
+            "traffic_unit": "bytes per launch (dram read + write, ncu --set full; profiles/r2_trace_traffic.md, null when the "
+                            "kernel sources changed since the capture)",
             "kernel": f"{dom[1]} ({dom[0]} batch)",
             "peak_source": (f"{peak_kind} HBM copy" if roof["bound"] == "hbm" else
                             f"148 SMs x 128 fp32 lanes x {sm_max_mhz:.0f} MHz (DESIGN.md)")}
 
+    # ---- later bounces and shuffled input of the headline scene: the regimes in which the rays are NOT already in
+    #      camera order (PAPER.md:294-299 measures secondary rays of every bounce)
+    by_bounce = {str(args.bounce): {"speedup_hcc": speed, "rays": n,
+                                    "trace_ms": {o: {b_: orders[o][b_]["trace_ms"] for b_ in ("diffuse", "shadow")} for o in orders}}}
+    shuffled = None
+    if world == 1 and not args.quick:
+        k_b = max(3, min(args.steps, 10))
+        for b_i in range(args.bounce + 1, args.bounce + 3):
+            set_bounce(sc, b_i)
+            o_b, s_b = compare(sc, k_b)
+            by_bounce[str(b_i)] = {"speedup_hcc": s_b, "rays": sc.n,
+                                   "trace_ms": {o: {b_: o_b[o][b_]["trace_ms"] for b_ in ("diffuse", "shadow")} for o in o_b}}
+        set_bounce(sc, args.bounce, shuffle=True)
+        o_s, s_s = compare(sc, k_b)
+        shuffled = {"speedup_hcc": s_s, "trace_ms": {o: {b_: o_s[o][b_]["trace_ms"] for b_ in ("diffuse", "shadow")} for o in o_s},
+                    "incl_ms_per_step": {o: o_s[o]["ms_per_step"] for o in o_s},
+                    "how": "the same two batches in a seeded random order (a wavefront renderer does not emit rays in camera order)"}
+        set_bounce(sc, args.bounce)
+        step(sc, hcc.ORDER_HCC)      # the hit buffers hold the unshuffled batches' results again (checked by the e2e leg)
+        hits_d, hits_s = sc.hits["diffuse"], sc.hits["shadow"]
+        (diffuse, _, _), (shadow, _, _) = sc.batches
+
     # ---- encode and sort at the batch size of configs 3/5 (the shadow batch tiled to ~33.5 M rays): the
     #      config-2 batches (1-2 M pairs) are launch- and latency-bound, so the HBM fractions that the
     #      north_star's 60 % bar is about are measured here (SURVEY.md §7 "hard parts", §8(d))
+    def med(fn, setup=None, k=7):
+        out = []
+        for i in range(k + 2):
+            if setup:
+                setup()
+            flush.zero_()
+            s0, e0 = ev(), ev()
+            s0.record(); fn(); e0.record()
+            torch.cuda.synchronize()
+            if i >= 2:
+                out.append(s0.elapsed_time(e0))
+        return float(np.median(out))
+
     large = None
     if world == 1 and not args.no_large_n:
         reps = max(1, (1 << 25) // n_s)
         big = shadow.repeat(reps, 1) if reps > 1 else shadow
         nb = big.shape[0]
-        keys_b = hcc.encode(big, cut)
-        keys_b0 = keys_b.clone()
-        ws_b = torch.empty(hcc.sort_workspace_bytes(nb, container), dtype=torch.uint8, device="cuda")
-        perm_b = torch.empty(nb, dtype=torch.int32, device="cuda")
 
-        def med(fn, setup=None, k=7):
-            out = []
-            for i in range(k + 2):
-                if setup:
-                    setup()
-                flush.zero_()
-                s0, e0 = ev(), ev()
-                s0.record(); fn(); e0.record()
-                torch.cuda.synchronize()
-                if i >= 2:
-                    out.append(s0.elapsed_time(e0))
-            return float(np.median(out))
+        def hbm_leg(ms, nbytes, **extra):
+            return {"ms": ms, "bound": "hbm", "achieved": nbytes / ms / 1e6, "peak": hbm_gbs, "unit": "GB/s",
+                    "frac": nbytes / ms / 1e6 / hbm_gbs, **extra}
+
+        def sort_leg(keys, bits_used, cb):
+            keys0 = keys.clone()
+            ws = torch.empty(hcc.sort_workspace_bytes(nb, cb), dtype=torch.uint8, device="cuda")
+            pm = torch.empty(nb, dtype=torch.int32, device="cuda")
+            ms = med(lambda: hcc.sort(keys, bits_used, perm=pm, workspace=ws), setup=lambda: keys.copy_(keys0))
+            p_ = (bits_used + 7) // 8
+            algo, real = sort_bytes(cb // 8, p_)
+            return hbm_leg(ms, nb * real, passes=p_, bytes_per_pair_moved=real, bytes_per_pair_survey=algo,
+                           frac_survey_bytes=nb * algo / ms / 1e6 / hbm_gbs)
+        keys_b = hcc.encode(big, cut)
         enc_ms = med(lambda: hcc.encode(big, cut, keys=keys_b))
-        sort_ms = med(lambda: hcc.sort(keys_b, info["bits_used"], perm=perm_b, workspace=ws_b), setup=lambda: keys_b.copy_(keys_b0))
+        tkb = 4 if w.key_bits <= 32 else 8
         tp_keys = hcc.encode_twopoint(big, bvh.scene_lo, bvh.scene_hi, w.key_bits)
         tp_ms = med(lambda: hcc.encode_twopoint(big, bvh.scene_lo, bvh.scene_hi, w.key_bits, keys=tp_keys))
-        tp_keys0 = tp_keys.clone()
-        tp_bits_used = 6 * (w.key_bits // 6)
-        tp_cb = 32 if w.key_bits <= 32 else 64
-        tp_passes = (tp_bits_used + 7) // 8
-        ws_t = torch.empty(hcc.sort_workspace_bytes(nb, tp_cb), dtype=torch.uint8, device="cuda")
-        perm_t = torch.empty(nb, dtype=torch.int32, device="cuda")
-        tp_sort_ms = med(lambda: hcc.sort(tp_keys, tp_bits_used, perm=perm_t, workspace=ws_t), setup=lambda: tp_keys.copy_(tp_keys0))
-        tp_sort_bytes = nb * (tp_cb // 8 + tp_passes * 2 * (tp_cb // 8 + 4))
-        kb = container // 8
-        eb, sb_ = nb * (32 + kb), nb * (kb + passes * 2 * (kb + 4))
-        tkb = 4 if w.key_bits <= 32 else 8
         large = {"rays": int(nb), "how": f"shadow batch tiled x{reps}",
-                 "encode": {"ms": enc_ms, "bound": "hbm", "achieved": eb / enc_ms / 1e6, "peak": hbm_gbs, "unit": "GB/s",
-                            "frac": eb / enc_ms / 1e6 / hbm_gbs,
-                            "alu_frac": nb * info["bits_used"] * OPS_BOX / (enc_ms * 1e-3) / 1e12 / (SM_COUNT * LANES_PER_SM * sm_max_mhz * 1e6 / 1e12)},
-                 "sort": {"ms": sort_ms, "bound": "hbm", "achieved": sb_ / sort_ms / 1e6, "peak": hbm_gbs, "unit": "GB/s",
-                          "frac": sb_ / sort_ms / 1e6 / hbm_gbs, "passes": passes},
-                 "sort_twopoint_keys": {"ms": tp_sort_ms, "bound": "hbm", "achieved": tp_sort_bytes / tp_sort_ms / 1e6, "peak": hbm_gbs,
-                                        "unit": "GB/s", "frac": tp_sort_bytes / tp_sort_ms / 1e6 / hbm_gbs, "passes": tp_passes,
-                                        "note": "well-spread Morton digits: the per-bit ballot path of the sort"},
-                 "encode_twopoint": {"ms": tp_ms, "bound": "hbm", "achieved": nb * (32 + tkb) / tp_ms / 1e6, "peak": hbm_gbs,
-                                     "unit": "GB/s", "frac": nb * (32 + tkb) / tp_ms / 1e6 / hbm_gbs}}
-        del big, keys_b, keys_b0, ws_b, perm_b, tp_keys, tp_keys0, ws_t, perm_t
+                 "encode": hbm_leg(enc_ms, nb * (32 + container // 8), box_tests_per_ray=info["bits_used"],
+                                   alu_frac=nb * info["bits_used"] * OPS_BOX / (enc_ms * 1e-3) / 1e12 / alu_peak),
+                 "sort": sort_leg(keys_b, info["bits_used"], container),
+                 "encode_twopoint": hbm_leg(tp_ms, nb * (32 + tkb)),
+                 "sort_twopoint_keys": sort_leg(tp_keys, 6 * (w.key_bits // 6), 32 if w.key_bits <= 32 else 64)}
+        # the paper's own MLHCC16 (8 x 8 entries, 16 slab tests per ray): SURVEY.md 8(d) expects
+        # codes of <= 16 tests to be HBM-bound
+        cut16 = hcc.select_cut_levels(bvh, sc.had, [8, 8], 16)
+        keys16 = hcc.encode(big, cut16)
+        e16 = med(lambda: hcc.encode(big, cut16, keys=keys16))
+        large["encode_mlhcc16"] = hbm_leg(e16, nb * (32 + 4), box_tests_per_ray=16,
+                                          alu_frac=nb * 16 * OPS_BOX / (e16 * 1e-3) / 1e12 / alu_peak)
+        del big, keys_b, tp_keys, keys16
         torch.cuda.empty_cache()
+
+    # ---- the other single-GPU configs of BASELINE.json at their stated sizes: one bounce of config 3 ("fig1") and
+    #      of config 5 ("large"), three orders each
+    others = None
+    if world == 1 and args.configs:
+        others = {}
+        for name in args.configs.split(","):
+            if name == args.workload:
+                continue
+            t_load = time.time()
+            so = load(name, 1.0)
+            set_bounce(so, 1)
+            t_load = time.time() - t_load
+            k_o = 3
+            ms_o, _, _ = timed(so, hcc.ORDER_HCC, k_o, 3)
+            o_o, s_o = compare(so, k_o)
+            sb = sort_bytes(so.info["container_bits"] // 8, (so.info["bits_used"] + 7) // 8)
+            others[name] = {"config": _config(args, so.w, so.n_d, so.n_s, l2="flushed between timed steps", workload=name),
+                            "value": so.n / ms_o / 1e3, "unit": UNIT, "ms_per_step": ms_o, "steps": k_o,
+                            "cut": {"widths": so.info["widths"], "bits_used": so.info["bits_used"], "cut_ms": so.cut_ms},
+                            "orders": o_o, "speedup_hcc": s_o,
+                            "sort_frac_of_hbm": {b_: nb_ * sb[1] / (o_o["hcc"][b_]["sort_ms"] * 1e-3) / 1e9 / hbm_gbs
+                                                 for b_, nb_ in (("diffuse", so.n_d), ("shadow", so.n_s))},
+                            "encode_frac_of_hbm": {b_: nb_ * (32 + so.info["container_bits"] // 8) / (o_o["hcc"][b_]["encode_ms"] * 1e-3) / 1e9 / hbm_gbs
+                                                   for b_, nb_ in (("diffuse", so.n_d), ("shadow", so.n_s))},
+                            "counters": counters(so) if args.counters_all else None,
+                            "input_generation_s": t_load}
+            del so
+            torch.cuda.empty_cache()
 
     # ---- studies, on request: f1 sort truncation, f2 lambda and
     #      ANC, f3 prefix path code (:116-128), f4 regular grid (:243)
     studies = None
     if args.studies and world == 1:
+        batches = sc.batches
+        hits = sc.hits
+        had = sc.had
+
         def med_ms(fn, setup=None, k=5):
-            out = []
-            for i in range(k + 1):
-                if setup:
-                    setup()
-                flush.zero_()
-                s0, e0 = ev(), ev()
-                s0.record(); fn(); e0.record()
-                torch.cuda.synchronize()
-                if i >= 1:
-                    out.append(s0.elapsed_time(e0))
-            return float(np.median(out))
+            return med(fn, setup, k)
 
         def run_order(make_keys, bits_used, bit_lo=0):
             """encode / sort / trace medians and ANC per batch for one key function (None = NoSort)."""
@@ -522,18 +698,7 @@ def run_ours(args):
                 sweep.append({"order": "hcc", "key_bits": kb, "K": K, "K_eff": i_s["K_eff"], "widths": i_s["widths"],
                               "bits_used": i_s["bits_used"], **run_order(hcc_keys(cut_s), i_s["bits_used"])})
         studies["sweep"] = sweep
-        # the same rays in a SHUFFLED input order (a wavefront renderer does not emit rays in camera order):
-        # the regime in which reordering has something to gain
-        saved = batches
-        g = torch.Generator(device="cuda").manual_seed(0x5EED)
-        batches = tuple((rays[torch.randperm(rays.shape[0], device="cuda", generator=g)].contiguous(), mode, name)
-                        for rays, mode, name in saved)
-        studies["orders_shuffled_input"] = {
-            "nosort": run_order(None, 0),
-            "twopoint": run_order(lambda rays, keys=None: hcc.encode_twopoint(rays, bvh.scene_lo, bvh.scene_hi, w.key_bits, keys=keys), tp_bits),
-            "hcc": run_order(hcc_keys(cut), info["bits_used"])}
-        batches = saved
-        step(hcc.ORDER_HCC)          # the hit buffers hold the unshuffled batches' results again (checked by the e2e leg)
+        step(sc, hcc.ORDER_HCC)
         studies["note"] = ("per batch medians of 5; grid = regular-grid tables of the same widths through the same encoder; "
                            "ppc = prefix path code with key_bits tests (upper-bound ordering, PAPER.md:128)")
 
@@ -549,7 +714,7 @@ def run_ours(args):
 
     def step_host():
         cur = torch.cuda.current_stream()
-        for _, mode, name in batches:
+        for _, mode, name in sc.batches:
             st = streams_h[name]
             st.wait_stream(cur)
             pipes_h[name].reorder_trace_host_async(bvh, cut, hcc.ORDER_HCC, rays_pin[name], hits_pin[name], mode,
@@ -566,16 +731,14 @@ def run_ours(args):
     e2e_ms = 0.0
     for _ in range(k_e2e):
         flush.zero_()
-        s, e = ev(), ev()
-        s.record()
+        s_, e_ = ev(), ev()
+        s_.record()
         step_host()
-        e.record()
+        e_.record()
         torch.cuda.synchronize()
-        e2e_ms += s.elapsed_time(e) / k_e2e
-    if world > 1:
-        t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+        e2e_ms += s_.elapsed_time(e_) / k_e2e
+    e2e_ms = max_over_ranks(e2e_ms)
+    step(sc, hcc.ORDER_HCC)
     assert torch.equal(hits_pin["shadow"].cuda(), hits_s) and torch.equal(hits_pin["diffuse"].cuda().view(torch.int32), hits_d.view(torch.int32))
     e2e = {"value": world * n / e2e_ms / 1e3, "unit": UNIT, "ms_per_step": e2e_ms,
            "h2d_bytes_per_step": 32 * n, "d2h_bytes_per_step": 16 * n_d + n_s}
@@ -604,12 +767,14 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
-            "config": _config(args, w, n_d, n_s, l2="flushed between timed steps (256 MiB write)"),
+            "config": _config(args, w, n_d, n_s, l2="flushed between timed steps (256 MiB write)", world=world),
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
             "roofline": roof, "cpu_baseline": cpu,
             "cut": {"widths": info["widths"], "K_eff": info["K_eff"], "bits_used": info["bits_used"],
-                    "container_bits": container, "cut_ms": cut_ms},
-            "orders": orders, "speedup_hcc": speed, "stages_roofline_hcc": stages, "stages_roofline_large_batch": large, "two_stream_step": overlapped, "studies": studies,
+                    "container_bits": container, "cut_ms": sc.cut_ms},
+            "orders": orders, "speedup_hcc": speed, "speedup_hcc_by_bounce": by_bounce, "shuffled_input": shuffled,
+            "stages_roofline_hcc": stages, "stages_roofline_large_batch": large, "two_stream_step": overlapped,
+            "strong_scaling": strong, "other_configs": others, "studies": studies,
             "diagnostics": diag,
             "paper_context": "RTX 3060, Breakfast: HCC 67.6 vs NoSort 37.4 vs TwoPoint 56.8 Mrays/s trace-only (PAPER.md:294-299); not comparable"}
     print(json.dumps(line))
@@ -632,9 +797,24 @@ def main():
     ap.add_argument("--res-scale", type=float, default=1.0, help="image scale of the workload (1.0 = the config's resolution)")
     ap.add_argument("--studies", action="store_true", help="add the NEXT-row studies: sort truncation, lambda/ANC, grid and PPC orders")
     ap.add_argument("--no-large-n", action="store_true", help="skip the large-batch encode/sort roofline leg")
+    ap.add_argument("--configs", default="fig1,large", help="comma list of further configs to run at their stated sizes (fig1,large): other_configs")
+    ap.add_argument("--counters-all", action="store_true", help="per-order trace counters for --configs too")
+    ap.add_argument("--quick", action="store_true", help="skip the later-bounce and shuffled-input legs")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # plain `python bench.py --gpus N`: start the N ranks ourselves (one process per GPU, NCCL)
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        return subprocess.call(cmd)
+    world_env = int(os.environ.get("WORLD_SIZE", "1"))
+    if world_env != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world_env}: launch with --nproc-per-node {args.gpus}")
     return run_reference(args) if args.impl == "reference" else run_ours(args)
 
 

@@ -117,7 +117,8 @@ HCC_API int32_t hcc_bvh_info(const hcc_bvh *bvh, uint32_t *n_nodes, uint32_t *n_
  * hcc_density: hierarchically accumulated density, Eq. 1 (:187):
  *   leaf  HAD = TC * SA;  internal  HAD = (HAD_left + HAD_right) + lambda * SA,
  *   SA = 2((dx*dy + dy*dz) + dz*dx), every operation one rounded fp32 operation.
- * density_dev: float32[n_nodes], written.  The paper uses lambda = 0.125 (:185, :276). */
+ * density_dev: float32[n_nodes], written (also used as the pass's own scratch, so calls on one BVH with
+ * different outputs may run concurrently).  The paper uses lambda = 0.125 (:185, :276). */
 HCC_API int32_t hcc_density(const hcc_bvh *bvh, float lambda, float *density_dev, void *stream);
 
 /* A cut handle with room for hierarchies of up to max_K finest-level nodes. */

@@ -127,9 +127,13 @@ __device__ __forceinline__ float surface_area(const hcc_node &nd) {
 }
 
 // Eq. 1, same bottom-up schedule.  Each node's value is computed exactly
-// once from its two final children, so the result does not depend on thread timing.
+// once from its two final children, so the result does not depend on thread timing.  The arrival
+// mark of an internal node lives in its own slot of the OUTPUT array (zeroed by hcc_density first): the
+// first child to arrive swaps 0 for HAD_PENDING and stops, the second finds the mark and writes the
+// value, so concurrent calls on one BVH (different outputs, different streams) share no scratch.
+constexpr uint32_t HAD_PENDING = 0xFFFFFFFFu;   // a NaN pattern no density takes
 __global__ void k_density(const hcc_node *__restrict__ nodes, const uint32_t *__restrict__ parent,
-                          uint32_t *flags, uint32_t n, float lambda, float *had) {
+                          uint32_t n, float lambda, float *had) {
     uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     hcc_node nd = nodes[i];
@@ -139,11 +143,11 @@ __global__ void k_density(const hcc_node *__restrict__ nodes, const uint32_t *__
     while (cur != 0u) {
         uint32_t p = parent[cur];
         __threadfence();
-        if (atomicAdd(&flags[p], 1u) == 0u) return;
+        if (atomicCAS(reinterpret_cast<uint32_t *>(had) + p, 0u, HAD_PENDING) == 0u) return;
         hcc_node pn = nodes[p];
         float hl = __ldcg(&had[pn.left_or_first]);
         float hr = __ldcg(&had[pn.left_or_first + 1u]);
-        had[p] = (hl + hr) + (lambda * surface_area(pn));
+        __stcg(&had[p], (hl + hr) + (lambda * surface_area(pn)));
         cur = p;
     }
 }
@@ -374,9 +378,9 @@ extern "C" int32_t hcc_density(const hcc_bvh *b, float lambda, float *density_de
     HCC_REQUIRE(aligned(density_dev, 16), HCC_ERR_BAD_ALIGNMENT, "hcc_density: density_dev not 16-byte aligned");
     HCC_REQUIRE(lambda >= 0.0f, HCC_ERR_INVALID_ARG, "hcc_density: lambda must be >= 0");
     cudaStream_t s = (cudaStream_t)stream;
-    HCC_CUDA_TRY(cudaMemsetAsync(b->d_flags, 0, sizeof(uint32_t) * (size_t)b->n_nodes, s));
+    HCC_CUDA_TRY(cudaMemsetAsync(density_dev, 0, sizeof(float) * (size_t)b->n_nodes, s));
     const uint32_t T = 256;
-    k_density<<<(b->n_nodes + T - 1) / T, T, 0, s>>>(b->d_nodes, b->d_parent, b->d_flags, b->n_nodes, lambda, density_dev);
+    k_density<<<(b->n_nodes + T - 1) / T, T, 0, s>>>(b->d_nodes, b->d_parent, b->n_nodes, lambda, density_dev);
     HCC_CUDA_TRY(cudaGetLastError());
     return HCC_OK;
 }

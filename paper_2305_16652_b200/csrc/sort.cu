@@ -333,16 +333,18 @@ static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t bit_l
     k_scan_hist<<<passes, RADIX, 0, s>>>(ctl, status, status_stride, n);
     const size_t dyn = (sizeof(KeyT) + sizeof(uint32_t)) * SORT_TILE;
     constexpr int SORT_THREADS = SortCfg<KeyT>::THREADS;
-    static bool attr_done = false;
-    if (!attr_done) {
+    // once per device and key width: the dynamic shared-memory limit and the resident CTAs per SM
+    static std::atomic<int> per_sm_cache[HCC_MAX_DEVICES];
+    const int dev = current_device();
+    int per_sm = per_sm_cache[dev].load(std::memory_order_acquire);
+    if (per_sm == 0) {
         HCC_CUDA_TRY(cudaFuncSetAttribute(k_onesweep<KeyT, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
         HCC_CUDA_TRY(cudaFuncSetAttribute(k_onesweep<KeyT, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
         HCC_CUDA_TRY(cudaFuncSetAttribute(k_onesweep<KeyT, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
         HCC_CUDA_TRY(cudaFuncSetAttribute(k_onesweep<KeyT, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
-        attr_done = true;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_onesweep<KeyT, false, true>, SORT_THREADS, dyn) != cudaSuccess || per_sm < 1) per_sm = 1;
+        per_sm_cache[dev].store(per_sm, std::memory_order_release);
     }
-    int per_sm = 1;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_onesweep<KeyT, false, true>, SORT_THREADS, dyn) != cudaSuccess || per_sm < 1) per_sm = 1;
     const uint32_t resident = (uint32_t)(sm_count() * per_sm);
     const uint32_t grid = tiles < resident ? tiles : resident;     // every CTA resident: the look-back cannot starve
     KeyT *kin = keys, *kout = keys_tmp;

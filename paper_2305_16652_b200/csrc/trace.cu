@@ -321,7 +321,10 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
                     const uint32_t rank = __popc(idle & lanes_below);
                     if (!have && rank < avail) {
                         const uint32_t j = w_next + rank;
-                        rid = perm ? ld_stream(perm + j) : j;
+                        // a sorted order is walked from its END: hierarchy cut codes carry their densest cut nodes in
+                        // the top bits, so the rays with the most traversal work start first and the kernel's tail
+                        // (the last rays running alone) is made of cheap ones; a warp's rays stay neighbours
+                        rid = perm ? ld_stream(perm + (n - 1u - j)) : j;
                         const float4 a = ld_stream4(rays + 2 * (size_t)rid), b = ld_stream4(rays + 2 * (size_t)rid + 1);
                         sts128(sa_slot, a);
                         sts128(sa_slot + 16u, b);

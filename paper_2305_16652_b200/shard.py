@@ -34,3 +34,15 @@ def gather_hits(local, n, group=None):
     parts = [torch.empty_like(pad) for _ in range(world)]
     dist.all_gather(parts, pad, group=group)
     return torch.cat([p[:s] for p, s in zip(parts, sizes)], 0)
+
+
+def sharded_reorder_trace(pipe, bvh, cut, order, rays, mode, rank, world, key_bits=32, hits=None, stream=None):
+    """This rank's share of one batch through the one-call hot path (hcc_reorder_trace): `rays` is the
+    WHOLE batch on this rank's device ([n, 8] float32, replicated like the BVH and the cut); the rank
+    encodes, sorts and traces rays[start:stop] only.  Returns (local hits, (start, stop)); the hits of
+    ray start + i are at local index i.  No collective: gather_hits is for a consumer that wants them
+    all in one place."""
+    start, stop = ray_shard(rays.shape[0], rank, world)
+    local = rays[start:stop]          # contiguous rows of 32 bytes: the slice keeps the 32-byte alignment
+    out = pipe.reorder_trace(bvh, cut, order, local, mode, hits=hits, key_bits=key_bits, stream=stream)
+    return out, (start, stop)

@@ -108,7 +108,10 @@ def test_select_cut_flat_any_K(hcc, dev_cases, name):
 
 
 # ------------------------------------------------------------------------------- (a2)
-ENC_REQUESTS = [(64, 32), (32, 32), (64, 64), (1024, 32), (4096, 64), (16384, 64), (256, 16), (48, 48), (1000, 48)]
+# (4096, 24) and (65536, 32) are six and eight levels of 4 (the hierarchies bench.py --studies sweeps); (16384, 48)
+# and (65536, 64) have level tables past the 160 KB that fit shared memory (the global-memory branch of the encoder)
+ENC_REQUESTS = [(64, 32), (32, 32), (64, 64), (1024, 32), (4096, 64), (16384, 64), (256, 16), (48, 48), (1000, 48),
+                (4096, 24), (65536, 32), (16384, 48), (65536, 64)]
 
 
 @pytest.mark.parametrize("name", ["tiny", "room_mid"])

@@ -168,6 +168,10 @@ def test_alg2_leaf_rule_fig7():
     cut_invariants(b.nodes, c, 7)
     # K larger than the number of leaves (9): the queue drains, every leaf is returned
     assert sorted(O.cut(b.nodes, had, 50).tolist()) == [1, 9, 10, 11, 12, 13, 14, 15, 16]
+    # "large enough" counts LEAVES below a node, not triangles (the subtree must be able to
+    # fill the next level's table with cut nodes): leaf 1 holds four triangles and still counts once
+    assert b.nodes["count"][1] == 4
+    assert O.subtree_leaves(b.nodes).tolist() == [9, 1, 8, 4, 4, 2, 2, 2, 2, 1, 1, 1, 1, 1, 1, 1, 1]
 
 
 def test_alg2_tie_break_lower_index():

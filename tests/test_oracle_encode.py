@@ -295,6 +295,14 @@ def test_twopoint_closed_forms():
         # only o.x in the upper half: the very first bit
         r = np.array([[0.75, 0, 0, 0, -3, 0, 0, np.inf]], np.float32)   # end x = 0
         assert int(O.encode_twopoint(r, lo, hi_, B)[0]) >> (6 * b - 1) == 1
+        # one coordinate in the upper half at a time: o.x o.y o.z t.x t.y t.z from the top bit down (DESIGN.md
+        # R10), so y and z cannot be swapped inside either triple.  The end point is o + 0.25 * d (e = 1).
+        top6 = lambda ray: int(O.encode_twopoint(np.array([ray], np.float32), lo, hi_, B)[0]) >> (6 * b - 6)
+        assert top6([0, 0.75, 0, 0, 0, -3, 0, np.inf]) == 0b010000      # o.y only (end y = 0)
+        assert top6([0, 0, 0.75, 0, 0, 0, -3, np.inf]) == 0b001000      # o.z only
+        assert top6([0, 0, 0, 0, 3, 0, 0, np.inf]) == 0b000100          # t.x only (end x = 0.75)
+        assert top6([0, 0, 0, 0, 0, 3, 0, np.inf]) == 0b000010          # t.y only
+        assert top6([0, 0, 0, 0, 0, 0, 3, np.inf]) == 0b000001          # t.z only
 
 
 def test_twopoint_monotone_and_range(room_small):

@@ -262,25 +262,7 @@ def test_alg3_discard_properties_on_a_real_bvh(tiny, widths):
 def test_alg3_discard_equals_retire_when_every_subtree_is_large():
     """On a perfect tree cut well above the leaves no popped node is too small: both variants agree."""
     depth = 7
-    n_nodes = 2 ** (depth + 1) - 1
-    # pre-order perfect binary tree with level-uniform boxes
-    nodes, tris = [None] * n_nodes, []
-    counter = [0]
-
-    def build(level, lo, hi):
-        i = counter[0]; counter[0] += 1
-        if level == depth:
-            nodes[i] = ((lo, 0, 0), (hi, 1, 1), len(tris), 1)
-            tris.append(np.zeros((3, 3), np.float32))
-            return i
-        nodes[i] = None
-        left = counter[0]
-        mid = 0.5 * (lo + hi)
-        build(level + 1, lo, mid)
-        build(level + 1, mid, hi)
-        nodes[i] = ((lo, 0, 0), (hi, 1, 1), left, 0)
-        return i
-    # children must be adjacent (right = left + 1): number breadth-first instead
+    # perfect binary tree with level-uniform boxes; children must be adjacent (right = left + 1): numbered breadth-first
     nodes = []
     width = 1
     for level in range(depth + 1):

@@ -73,3 +73,39 @@ def test_sharded_path_equals_single_process(tiny):
     assert np.array_equal(full[:, 0], t.astype(np.float64))
     assert np.array_equal(full[:, 1], prim.astype(np.float64))
     assert np.array_equal(keys_full.astype(np.uint64), oracle.encode_hcc(rays, b.nodes, tables))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("world", [1, 3])
+def test_sharded_product_path_on_one_gpu(world, tiny):
+    """The code path bench.py --gpus N runs per rank (shard.sharded_reorder_trace -> hcc_reorder_trace on the
+    rank's contiguous range), on the single GPU of the test box: the shards of every rank of a `world`-rank job,
+    run one after the other, tile the batch and reproduce the unsharded hits bit for bit; with a one-rank
+    process group gather_hits returns the same tensor."""
+    import torch
+    import torch.distributed as dist
+    import paper_2305_16652_b200 as hcc
+    from paper_2305_16652_b200.shard import gather_hits, sharded_reorder_trace
+    b = tiny.bvh
+    bvh = hcc.Bvh(b.nodes, b.tris, b.prim_idx)
+    cut = hcc.select_cut(bvh, hcc.density(bvh), 64, 32)
+    for rays_h, mode in ((tiny.diffuse[:4001], hcc.TRACE_CLOSEST), (tiny.shadow[:8003], hcc.TRACE_ANY)):
+        rays = torch.from_numpy(rays_h).cuda()
+        n = rays.shape[0]
+        pipe = hcc.Pipeline(n, 64)
+        whole = hcc.trace(bvh, rays, None, mode)
+        parts, spans = [], []
+        for rank in range(world):
+            local, span = sharded_reorder_trace(pipe, bvh, cut, hcc.ORDER_HCC, rays, mode, rank, world)
+            parts.append(local.clone())
+            spans.append(span)
+        assert spans[0][0] == 0 and spans[-1][1] == n and all(a[1] == c[0] for a, c in zip(spans, spans[1:]))
+        assert torch.equal(torch.cat(parts, 0).view(torch.uint8), whole.view(torch.uint8))
+    if world == 1:
+        os.environ["MASTER_ADDR"] = "127.0.0.1"
+        os.environ["MASTER_PORT"] = str(_free_port())
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+        try:
+            assert torch.equal(gather_hits(parts[0], n).view(torch.uint8), whole.view(torch.uint8))
+        finally:
+            dist.destroy_process_group()
