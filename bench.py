@@ -5,8 +5,10 @@
 One STEP = one pass of the whole per-batch hot path (Figure 11) over one
 bounce of BASELINE.json config 2 ("room": 64,012 triangles, 512x512x4 spp): the diffuse batch
 (1,048,576 closest-hit rays) and the shadow batch (2,097,152 any-hit rays), each
-key-computed (hcc_encode), sorted (hcc_sort) and traced through the sorted indices (hcc_trace)
-in ONE C-ABI call, hcc_reorder_trace.  Metric: secondary Mrays/s INCLUDING encode + sort.
+key-computed (hcc_encode), sorted (hcc_sort) and traced through the sorted indices (hcc_trace),
+both in ONE C-ABI call, hcc_reorder_trace_pair (the kernels of the call are chained by programmatic
+dependent launch; the per-stage split comes from separate, event-ordered hcc_reorder_trace calls).
+Metric: secondary Mrays/s INCLUDING encode + sort.
 The same rays are also run in the NoSort and TwoPoint orders and the
 per-stage split, speed-ups, ANC and roofline fractions are reported in the
 JSON line.  The cut (hcc_density + hcc_select_cut) is a once-per-scene pre-process in the
@@ -324,8 +326,9 @@ def run_ours(args):
                    "shadow": torch.empty(sc.n_s, dtype=torch.uint8, device="cuda")}
 
     def step(sc, order):
-        for rays, mode, name in sc.batches:
-            sc.pipe.reorder_trace(sc.bvh, sc.cut, order, rays, mode, hits=sc.hits[name], key_bits=sc.w.key_bits)
+        """One step = both batches of the bounce through the hot path, ONE C-ABI call (hcc_reorder_trace_pair)."""
+        (ra, ma, na), (rb, mb, nb_) = sc.batches
+        sc.pipe.reorder_trace_pair(sc.bvh, sc.cut, order, ra, ma, sc.hits[na], rb, mb, sc.hits[nb_], key_bits=sc.w.key_bits)
 
     def timed(sc, order, steps, warmup, per_stage=False):
         for _ in range(warmup):
@@ -341,11 +344,13 @@ def run_ours(args):
             flush.zero_()                       # L2 flush, outside the event bracket
             s_.record()
             if per_stage:
+                sc.pipe.set_timing(True)
                 for rays, mode, name in sc.batches:
                     sc.pipe.reorder_trace(sc.bvh, sc.cut, order, rays, mode, hits=sc.hits[name], key_bits=sc.w.key_bits)
                     ms = sc.pipe.stage_ms()
                     for k in stage[name]:
                         stage[name][k] += ms[k] / steps
+                sc.pipe.set_timing(False)
             else:
                 step(sc, order)
             e_.record()
@@ -743,8 +748,8 @@ def run_ours(args):
     e2e = {"value": world * n / e2e_ms / 1e3, "unit": UNIT, "ms_per_step": e2e_ms,
            "h2d_bytes_per_step": 32 * n, "d2h_bytes_per_step": 16 * n_d + n_s}
 
-    # kernels launched per step: per batch 1 key kernel + (histogram + scan + one per digit) + 1 trace
-    launches_per_step = 2 * (1 + (2 + passes) + 1)
+    # kernels launched per step: per batch 1 key kernel + (init + histogram + scan + one per digit) + 1 trace
+    launches_per_step = 2 * (1 + (3 + passes) + 1)
 
     if rank != 0:
         if world > 1:

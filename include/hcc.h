@@ -306,11 +306,25 @@ HCC_API int32_t hcc_reorder_trace_host(hcc_pipeline *p, const hcc_bvh *bvh, cons
 HCC_API int32_t hcc_reorder_trace_host_async(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
                                      uint32_t key_bits, const float *rays_host, uint64_t n, int32_t mode,
                                      void *hits_host, void *stream);
+/* Both batches of one bounce in one call: batch a (say the diffuse rays, HCC_TRACE_CLOSEST) and batch b (the
+ * shadow rays, HCC_TRACE_ANY) go through the same three kernels as in hcc_reorder_trace, a first.  The kernels
+ * are chained by programmatic dependent launch and batch b's chain starts WITHOUT waiting for batch a's trace
+ * kernel: b is encoded and sorted while a's traversal runs out, so both batches must be complete in memory
+ * when the call is made (no kernel enqueued in between can have produced b's rays: there is none).  Results
+ * are those of two hcc_reorder_trace calls.  Either n may be 0.  Per-stage timing is not recorded. */
+HCC_API int32_t hcc_reorder_trace_pair(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
+                               uint32_t key_bits, const float *rays_a_dev, uint64_t n_a, int32_t mode_a,
+                               void *hits_a_dev, const float *rays_b_dev, uint64_t n_b, int32_t mode_b,
+                               void *hits_b_dev, void *stream);
 /* Waits until the pipeline's last enqueued call has finished. */
 HCC_API int32_t hcc_pipeline_synchronize(hcc_pipeline *p);
-/* Device time of the stages of the pipeline's last call, from CUDA events recorded on its
- * stream between the stages: ms[0] encode, [1] sort, [2] trace, [3] host->device copy,
- * [4] device->host copy (3, 4 = 0 for the device form).  Waits for that call to finish. */
+/* Per-stage timing: with enable != 0 every later hcc_reorder_trace(_host) call records CUDA events on its
+ * stream between the stages (this orders the stages completely: no kernel of a call overlaps the next one's
+ * prologue).  Off by default. */
+HCC_API int32_t hcc_pipeline_set_timing(hcc_pipeline *p, uint32_t enable);
+/* Device time of the stages of the pipeline's last timed call: ms[0] encode, [1] sort, [2] trace,
+ * [3] host->device copy, [4] device->host copy (3, 4 = 0 for the device form).  Waits for that call to
+ * finish.  HCC_ERR_INVALID_ARG if the last call was not timed (hcc_pipeline_set_timing). */
 HCC_API int32_t hcc_pipeline_stage_ms(hcc_pipeline *p, float ms[5]);
 
 /* ANC, "average number of codes per warp" (Table 7): for every group of 32

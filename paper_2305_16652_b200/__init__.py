@@ -55,6 +55,8 @@ _SIGNATURES = {
     "hcc_reorder_trace": [_vp, _vp, _vp, _i32, _u32, _vp, _u64, _i32, _vp, _vp, _vp],
     "hcc_reorder_trace_host": [_vp, _vp, _vp, _i32, _u32, _vp, _u64, _i32, _vp, _vp],
     "hcc_reorder_trace_host_async": [_vp, _vp, _vp, _i32, _u32, _vp, _u64, _i32, _vp, _vp],
+    "hcc_reorder_trace_pair": [_vp, _vp, _vp, _i32, _u32, _vp, _u64, _i32, _vp, _vp, _u64, _i32, _vp, _vp],
+    "hcc_pipeline_set_timing": [_vp, _u32],
     "hcc_pipeline_synchronize": [_vp],
     "hcc_pipeline_stage_ms": [_vp, _vp],
     "hcc_trace_stats": [_vp, _vp, _u64, _vp, _i32, _vp, _vp, _vp],
@@ -391,6 +393,18 @@ class Pipeline:
                                        int(key_bits), _rays_dev(rays), n, int(mode), _vp(hits.data_ptr()), po,
                                        _stream(stream)))
         return hits
+
+    def reorder_trace_pair(self, bvh, cut, order, rays_a, mode_a, hits_a, rays_b, mode_b, hits_b, key_bits=32, stream=None):
+        """hcc_reorder_trace_pair: both batches of one bounce in one call (b's keys and sort overlap a's traversal)."""
+        _check(lib().hcc_reorder_trace_pair(self._h, bvh._h, _vp(0) if cut is None else cut._h, int(order), int(key_bits),
+                                            _rays_dev(rays_a), rays_a.shape[0], int(mode_a), _vp(hits_a.data_ptr()),
+                                            _rays_dev(rays_b), rays_b.shape[0], int(mode_b), _vp(hits_b.data_ptr()),
+                                            _stream(stream)))
+        return hits_a, hits_b
+
+    def set_timing(self, enable=True):
+        """hcc_pipeline_set_timing: record the per-stage events of later calls (stage_ms)."""
+        _check(lib().hcc_pipeline_set_timing(self._h, 1 if enable else 0))
 
     def reorder_trace_host(self, bvh, cut, order, rays_host, hits_host, mode=TRACE_CLOSEST, key_bits=32,
                            stream=None):

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <stdlib.h>
 
 #include <atomic>
 
@@ -53,6 +54,45 @@ inline int sm_count() {
 }
 
 inline uint64_t round_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
+
+// ---- programmatic dependent launch (sm_90+).  The kernels of one library call form a chain: all but the
+// first are launched with the programmatic-stream-serialization attribute, so a kernel may become resident
+// while its predecessor still runs; it calls pdl_wait() before it touches anything a predecessor wrote (or
+// may still read) and pdl_trigger() only AFTER that wait.  Rule of the chain: a kernel that is launched has
+// seen its predecessor pass its own wait, so everything before the predecessor is complete; only the
+// predecessor itself may still run.  The FIRST kernel of a call is a plain launch (LK_FIRST): ordered after
+// everything enqueued on the stream before it.  LK_OVERLAP is for hcc_reorder_trace_pair only: the first
+// kernel of the second batch's chain is a dependent launch that does NOT wait, so the chain runs while the
+// first batch's traversal kernel drains.  HCC_NO_PDL=1 in the environment makes every launch a plain one.
+enum LaunchKind { LK_FIRST = 0, LK_CHAIN = 1, LK_OVERLAP = 2 };
+
+inline bool pdl_enabled() {
+    static const bool on = [] { const char *e = getenv("HCC_NO_PDL"); return !(e && e[0] == '1'); }();
+    return on;
+}
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_k(LaunchKind kind, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = (kind != LK_FIRST && pdl_enabled()) ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+// does the first kernel of a chain launched as `kind` call pdl_wait()?  (a plain launch needs no wait, but the call is a
+// no-op there; LK_OVERLAP must not wait - unless dependent launches are off, then it is a plain launch anyway)
+inline int kind_waits(LaunchKind kind) { return kind == LK_OVERLAP ? 0 : 1; }
+
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+#endif
 
 // Traversal grid (bvh.cu, trace.cu): child boxes are stored as 15-bit cell indices of a
 // uniform grid over the root box, rounded outwards and padded by one cell.
@@ -114,4 +154,16 @@ struct hcc_cut {
 // stage entry points implemented in the other translation units
 namespace hcc {
 int32_t launch_build_tables(const hcc_bvh *bvh, const float *had, hcc_cut *cut, cudaStream_t s);
+// The hot-path stages as hcc_reorder_trace chains them; `kind` is how the stage's first kernel is launched.
+int32_t encode_launch(const float *rays_dev, uint64_t n, const hcc_cut *cut, void *keys_dev, cudaStream_t s, LaunchKind kind);
+int32_t encode_twopoint_launch(const float *rays_dev, uint64_t n, const float scene_lo[3], const float scene_hi[3],
+                               uint32_t key_bits, void *keys_dev, cudaStream_t s, LaunchKind kind);
+// also_zero: two words the sort's first kernel zeroes besides its own control region (the trace work counter), or NULL
+int32_t sort_launch(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bit_lo, uint32_t bit_hi, uint32_t *perm_dev,
+                    void *workspace_dev, uint64_t workspace_bytes, cudaStream_t s, uint32_t *also_zero, LaunchKind kind);
+uint32_t *trace_take_slot(const hcc_bvh *bvh);
+// armed_slot: a work counter already zeroed by a kernel earlier in the chain (the trace kernel is then a chained
+// launch), or NULL (then a one-warp kernel launched as `kind` zeroes a fresh one first)
+int32_t trace_launch(const char *who, const hcc_bvh *bvh, const float *rays_dev, uint64_t n, const uint32_t *perm_dev, int32_t mode,
+                     void *hits_dev, unsigned long long *stats_dev, cudaStream_t s, uint32_t *armed_slot, LaunchKind kind);
 }

@@ -93,9 +93,11 @@ constexpr int ENC_THREADS_MAX = 1024;   // one big CTA per SM when the staged ta
 template <typename KeyT>
 __global__ void __launch_bounds__(ENC_THREADS_MAX)
 k_encode_hcc(const float4 *__restrict__ rays, uint64_t n, const CutDev cut, uint32_t smem_entries,
-             KeyT *__restrict__ keys) {
+             KeyT *__restrict__ keys, int wait) {
     extern __shared__ ulonglong2 s_box[];
     const ulonglong2 *g_box = reinterpret_cast<const ulonglong2 *>(cut.boxes);
+    if (wait) pdl_wait();
+    pdl_trigger();
     for (uint32_t i = threadIdx.x; i < 2u * smem_entries; i += blockDim.x) s_box[i] = g_box[i];
     __syncthreads();
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
@@ -146,7 +148,9 @@ __device__ __forceinline__ uint32_t quantise(float p, float lo, float hi, float 
 template <typename KeyT>
 __global__ void __launch_bounds__(ENC_THREADS)
 k_encode_twopoint(const float4 *__restrict__ rays, uint64_t n, float3 lo, float3 hi, float len, uint32_t b,
-                  KeyT *__restrict__ keys) {
+                  KeyT *__restrict__ keys, int wait) {
+    if (wait) pdl_wait();
+    pdl_trigger();
     const uint64_t stride = (uint64_t)gridDim.x * ENC_THREADS;
     const float scale = (float)(1u << b);
     const uint32_t qmax = (1u << b) - 1u;
@@ -177,6 +181,8 @@ template <typename KeyT>
 __global__ void __launch_bounds__(ENC_THREADS)
 k_encode_ppc(const float4 *__restrict__ rays, uint64_t n, const float4 *__restrict__ nodes, uint32_t bits,
              KeyT *__restrict__ keys) {
+    pdl_wait();
+    pdl_trigger();
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     for (uint64_t ri = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; ri < n; ri += stride) {
         float4 a, b;
@@ -208,26 +214,55 @@ k_encode_ppc(const float4 *__restrict__ rays, uint64_t n, const float4 *__restri
     }
 }
 
-static int grid_for(const void *kernel, size_t smem, uint64_t n, int threads = ENC_THREADS) {
+// CTAs per SM of `kernel` at (threads, smem), queried once per device and configuration
+static int ctas_per_sm(const void *kernel, int threads, size_t smem) {
+    struct Entry { const void *k; int dev, threads; size_t smem; int per_sm; };
+    static Entry cache[32];
+    static std::atomic<int> used{0};
+    const int dev = current_device();
+    const int n = used.load(std::memory_order_acquire);
+    for (int i = 0; i < n; ++i)
+        if (cache[i].k == kernel && cache[i].dev == dev && cache[i].threads == threads && cache[i].smem == smem) return cache[i].per_sm;
     int per_sm = 1;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+    static std::atomic_flag busy = ATOMIC_FLAG_INIT;
+    if (!busy.test_and_set(std::memory_order_acquire)) {       // best effort: a lost race only repeats the query
+        const int m = used.load(std::memory_order_relaxed);
+        if (m < 32) { cache[m] = Entry{kernel, dev, threads, smem, per_sm}; used.store(m + 1, std::memory_order_release); }
+        busy.clear(std::memory_order_release);
+    }
+    return per_sm;
+}
+
+static int grid_for(const void *kernel, size_t smem, uint64_t n, int threads = ENC_THREADS) {
+    const int per_sm = ctas_per_sm(kernel, threads, smem);
     uint64_t want = (n + threads - 1) / threads;
     uint64_t cap = (uint64_t)sm_count() * (uint64_t)per_sm;
     return (int)(want < cap ? want : cap);
+}
+
+// the dynamic shared-memory limit of the HCC encoder, raised once per device
+template <typename KeyT>
+static cudaError_t encode_attr(size_t budget) {
+    static std::atomic<int> done[HCC_MAX_DEVICES];
+    const int dev = current_device();
+    if (done[dev].load(std::memory_order_acquire)) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(k_encode_hcc<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget);
+    if (e == cudaSuccess) done[dev].store(1, std::memory_order_release);
+    return e;
 }
 
 }  // namespace hcc
 
 using namespace hcc;
 
-extern "C" int32_t hcc_encode(const float *rays_dev, uint64_t n, const hcc_cut *cut, void *keys_dev, void *stream) {
+int32_t hcc::encode_launch(const float *rays_dev, uint64_t n, const hcc_cut *cut, void *keys_dev, cudaStream_t s, LaunchKind kind) {
     HCC_REQUIRE(cut && cut->valid, HCC_ERR_INVALID_ARG, "hcc_encode: the cut handle holds no selection");
     if (n == 0) return HCC_OK;
     HCC_REQUIRE(rays_dev && keys_dev, HCC_ERR_INVALID_ARG, "hcc_encode: NULL argument");
     HCC_REQUIRE(aligned(rays_dev, 32) && aligned(keys_dev, 16), HCC_ERR_BAD_ALIGNMENT,
                 "hcc_encode: rays need 32-byte, keys 16-byte alignment");
     HCC_REQUIRE(n < (1ull << 32), HCC_ERR_UNSUPPORTED, "hcc_encode: n >= 2^32");
-    cudaStream_t s = (cudaStream_t)stream;
     const CutDev &d = cut->dev;
     // stage whole levels, top down, while they fit in 160 KB (leaves room for 1 CTA/SM at worst)
     const size_t budget = 160 * 1024;
@@ -241,26 +276,30 @@ extern "C" int32_t hcc_encode(const float *rays_dev, uint64_t n, const hcc_cut *
     const int threads = smem > 100 * 1024 ? 1024 : smem > 48 * 1024 ? 512 : ENC_THREADS;
     if (cut->container_bits == 32) {
         auto kern = k_encode_hcc<uint32_t>;
-        HCC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget));
-        kern<<<grid_for((const void *)kern, smem, n, threads), threads, smem, s>>>((const float4 *)rays_dev, n, d, smem_entries, (uint32_t *)keys_dev);
+        HCC_CUDA_TRY(encode_attr<uint32_t>(budget));
+        HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, smem, n, threads)), dim3(threads), smem, s,
+                                (const float4 *)rays_dev, n, d, smem_entries, (uint32_t *)keys_dev, kind_waits(kind)));
     } else {
         auto kern = k_encode_hcc<unsigned long long>;
-        HCC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget));
-        kern<<<grid_for((const void *)kern, smem, n, threads), threads, smem, s>>>((const float4 *)rays_dev, n, d, smem_entries, (unsigned long long *)keys_dev);
+        HCC_CUDA_TRY(encode_attr<unsigned long long>(budget));
+        HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, smem, n, threads)), dim3(threads), smem, s,
+                                (const float4 *)rays_dev, n, d, smem_entries, (unsigned long long *)keys_dev, kind_waits(kind)));
     }
-    HCC_CUDA_TRY(cudaGetLastError());
     return HCC_OK;
 }
 
-extern "C" int32_t hcc_encode_twopoint(const float *rays_dev, uint64_t n, const float scene_lo[3], const float scene_hi[3],
-                                       uint32_t key_bits, void *keys_dev, void *stream) {
+extern "C" int32_t hcc_encode(const float *rays_dev, uint64_t n, const hcc_cut *cut, void *keys_dev, void *stream) {
+    return encode_launch(rays_dev, n, cut, keys_dev, (cudaStream_t)stream, LK_FIRST);
+}
+
+int32_t hcc::encode_twopoint_launch(const float *rays_dev, uint64_t n, const float scene_lo[3], const float scene_hi[3],
+                                    uint32_t key_bits, void *keys_dev, cudaStream_t s, LaunchKind kind) {
     HCC_REQUIRE(key_bits == 16 || key_bits == 24 || key_bits == 32 || key_bits == 48 || key_bits == 64,
                 HCC_ERR_INVALID_ARG, "hcc_encode_twopoint: key_bits must be 16, 24, 32, 48 or 64");
     if (n == 0) return HCC_OK;
     HCC_REQUIRE(rays_dev && keys_dev && scene_lo && scene_hi, HCC_ERR_INVALID_ARG, "hcc_encode_twopoint: NULL argument");
     HCC_REQUIRE(aligned(rays_dev, 32) && aligned(keys_dev, 16), HCC_ERR_BAD_ALIGNMENT,
                 "hcc_encode_twopoint: rays need 32-byte, keys 16-byte alignment");
-    cudaStream_t s = (cudaStream_t)stream;
     float3 lo = make_float3(scene_lo[0], scene_lo[1], scene_lo[2]);
     float3 hi = make_float3(scene_hi[0], scene_hi[1], scene_hi[2]);
     float e = fmaxf(fmaxf(hi.x - lo.x, hi.y - lo.y), hi.z - lo.z);
@@ -268,13 +307,19 @@ extern "C" int32_t hcc_encode_twopoint(const float *rays_dev, uint64_t n, const 
     uint32_t b = key_bits / 6u;
     if (key_bits <= 32) {
         auto kern = k_encode_twopoint<uint32_t>;
-        kern<<<grid_for((const void *)kern, 0, n), ENC_THREADS, 0, s>>>((const float4 *)rays_dev, n, lo, hi, len, b, (uint32_t *)keys_dev);
+        HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, 0, n)), dim3(ENC_THREADS), 0, s,
+                                (const float4 *)rays_dev, n, lo, hi, len, b, (uint32_t *)keys_dev, kind_waits(kind)));
     } else {
         auto kern = k_encode_twopoint<unsigned long long>;
-        kern<<<grid_for((const void *)kern, 0, n), ENC_THREADS, 0, s>>>((const float4 *)rays_dev, n, lo, hi, len, b, (unsigned long long *)keys_dev);
+        HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, 0, n)), dim3(ENC_THREADS), 0, s,
+                                (const float4 *)rays_dev, n, lo, hi, len, b, (unsigned long long *)keys_dev, kind_waits(kind)));
     }
-    HCC_CUDA_TRY(cudaGetLastError());
     return HCC_OK;
+}
+
+extern "C" int32_t hcc_encode_twopoint(const float *rays_dev, uint64_t n, const float scene_lo[3], const float scene_hi[3],
+                                       uint32_t key_bits, void *keys_dev, void *stream) {
+    return encode_twopoint_launch(rays_dev, n, scene_lo, scene_hi, key_bits, keys_dev, (cudaStream_t)stream, LK_FIRST);
 }
 
 extern "C" int32_t hcc_encode_ppc(const hcc_bvh *bvh, const float *rays_dev, uint64_t n, uint32_t key_bits, void *keys_dev,
@@ -291,10 +336,10 @@ extern "C" int32_t hcc_encode_ppc(const hcc_bvh *bvh, const float *rays_dev, uin
     const float4 *nodes = reinterpret_cast<const float4 *>(bvh->d_nodes);
     if (key_bits <= 32) {
         auto kern = k_encode_ppc<uint32_t>;
-        kern<<<grid_for((const void *)kern, 0, n), ENC_THREADS, 0, s>>>((const float4 *)rays_dev, n, nodes, key_bits, (uint32_t *)keys_dev);
+        HCC_CUDA_TRY(launch_k(LK_FIRST, kern, dim3(grid_for((const void *)kern, 0, n)), dim3(ENC_THREADS), 0, s, (const float4 *)rays_dev, n, nodes, key_bits, (uint32_t *)keys_dev));
     } else {
         auto kern = k_encode_ppc<unsigned long long>;
-        kern<<<grid_for((const void *)kern, 0, n), ENC_THREADS, 0, s>>>((const float4 *)rays_dev, n, nodes, key_bits, (unsigned long long *)keys_dev);
+        HCC_CUDA_TRY(launch_k(LK_FIRST, kern, dim3(grid_for((const void *)kern, 0, n)), dim3(ENC_THREADS), 0, s, (const float4 *)rays_dev, n, nodes, key_bits, (unsigned long long *)keys_dev));
     }
     HCC_CUDA_TRY(cudaGetLastError());
     return HCC_OK;

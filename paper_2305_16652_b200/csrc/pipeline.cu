@@ -12,13 +12,16 @@ struct hcc_pipeline {
     uint32_t container_bits_max;
     bool host_staging;
     void *d_keys;
-    uint32_t *d_perm;
+    uint32_t *d_perm[2];   // alternate per call: a call's sort may run while the previous call's trace still reads its perm
+    uint32_t calls;        // calls made
+    cudaStream_t last_stream;
+    bool timing;           // record the per-stage events (hcc_pipeline_set_timing)
     void *d_ws;
     uint64_t ws_bytes;
     float *d_rays;      // host-buffer form only
     void *d_hits;       // host-buffer form only
     cudaEvent_t ev[6];  // h2d start, encode start, sort start, trace start, trace end, d2h end
-    bool timed, timed_host;
+    bool timed, timed_host, host_pending;
     uint32_t sort_skip_bits;   // low key bits the sort leaves unordered (hcc_sort_range)
 };
 
@@ -50,7 +53,8 @@ using namespace hcc;
 extern "C" int32_t hcc_pipeline_destroy(hcc_pipeline *p) {
     if (!p) return HCC_OK;
     cudaFree(p->d_keys);
-    cudaFree(p->d_perm);
+    cudaFree(p->d_perm[0]);
+    cudaFree(p->d_perm[1]);
     cudaFree(p->d_ws);
     cudaFree(p->d_rays);
     cudaFree(p->d_hits);
@@ -75,7 +79,8 @@ extern "C" int32_t hcc_pipeline_create(uint64_t n_max, uint32_t container_bits_m
     int32_t rc = hcc_sort_workspace_bytes(n_max, container_bits_max, &p->ws_bytes);
     if (rc != HCC_OK) { delete p; return rc; }
     cudaError_t e = cudaMalloc(&p->d_keys, (size_t)(container_bits_max / 8) * n_max);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&p->d_perm, sizeof(uint32_t) * n_max);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&p->d_perm[0], sizeof(uint32_t) * n_max);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&p->d_perm[1], sizeof(uint32_t) * n_max);
     if (e == cudaSuccess) e = cudaMalloc(&p->d_ws, p->ws_bytes);
     if (e == cudaSuccess && p->host_staging) e = cudaMalloc((void **)&p->d_rays, 32 * n_max);
     if (e == cudaSuccess && p->host_staging) e = cudaMalloc(&p->d_hits, 16 * n_max);
@@ -96,44 +101,89 @@ extern "C" int32_t hcc_pipeline_set_sort_skip_bits(hcc_pipeline *p, uint32_t bit
     return HCC_OK;
 }
 
-extern "C" int32_t hcc_reorder_trace(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
-                                     uint32_t key_bits, const float *rays_dev, uint64_t n, int32_t mode,
-                                     void *hits_dev, uint32_t *perm_out_dev, void *stream) {
-    HCC_REQUIRE(p && bvh, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: NULL handle");
+extern "C" int32_t hcc_pipeline_set_timing(hcc_pipeline *p, uint32_t enable) {
+    HCC_REQUIRE(p, HCC_ERR_INVALID_ARG, "hcc_pipeline_set_timing: NULL pipeline");
+    p->timing = enable != 0;
+    return HCC_OK;
+}
+
+// One batch: key kernel -> sort kernels -> trace kernel as one chain of dependent launches (common.cuh).  `first` is how
+// the chain's first kernel is launched; `events` records the per-stage events between the stages.
+static int32_t run_chain(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order, uint32_t key_bits,
+                         const float *rays_dev, uint64_t n, int32_t mode, void *hits_dev, uint32_t *perm, cudaStream_t s,
+                         LaunchKind first, bool events) {
     HCC_REQUIRE(order == HCC_ORDER_NOSORT || order == HCC_ORDER_TWOPOINT || order == HCC_ORDER_HCC, HCC_ERR_INVALID_ARG,
                 "hcc_reorder_trace: unknown order %d", order);
     HCC_REQUIRE(n <= p->n_max, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: n exceeds the pipeline's n_max");
-    cudaStream_t s = (cudaStream_t)stream;
-    uint32_t *perm = perm_out_dev ? perm_out_dev : p->d_perm;
-    int32_t rc = HCC_OK;
-    p->timed = false;
-    HCC_CUDA_TRY(cudaEventRecord(p->ev[1], s));
+    HCC_REQUIRE(mode == HCC_TRACE_CLOSEST || mode == HCC_TRACE_ANY, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: unknown mode %d", mode);
     uint32_t container = 32, bits_used = 0;
     if (order == HCC_ORDER_HCC) {
         HCC_REQUIRE(cut && cut->valid, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: order HCC needs a selected cut");
         container = cut->container_bits;
         bits_used = cut->dev.bits_used;
-        HCC_REQUIRE(container <= p->container_bits_max, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: 64-bit keys in a 32-bit pipeline");
-        rc = hcc_encode(rays_dev, n, cut, p->d_keys, stream);
     } else if (order == HCC_ORDER_TWOPOINT) {
         container = key_bits <= 32 ? 32u : 64u;
         bits_used = 6u * (key_bits / 6u);
-        HCC_REQUIRE(container <= p->container_bits_max, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: 64-bit keys in a 32-bit pipeline");
-        rc = hcc_encode_twopoint(rays_dev, n, bvh->scene_lo, bvh->scene_hi, key_bits, p->d_keys, stream);
     }
+    HCC_REQUIRE(container <= p->container_bits_max, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: 64-bit keys in a 32-bit pipeline");
+    int32_t rc = HCC_OK;
+    if (events) HCC_CUDA_TRY(cudaEventRecord(p->ev[1], s));
+    if (order == HCC_ORDER_HCC) rc = encode_launch(rays_dev, n, cut, p->d_keys, s, first);
+    else if (order == HCC_ORDER_TWOPOINT) rc = encode_twopoint_launch(rays_dev, n, bvh->scene_lo, bvh->scene_hi, key_bits, p->d_keys, s, first);
     if (rc != HCC_OK) return rc;
-    HCC_CUDA_TRY(cudaEventRecord(p->ev[2], s));
-    if (order != HCC_ORDER_NOSORT) {
+    if (events) HCC_CUDA_TRY(cudaEventRecord(p->ev[2], s));
+    uint32_t *slot = nullptr;
+    if (order != HCC_ORDER_NOSORT && n != 0) {
         const uint32_t lo = p->sort_skip_bits < bits_used ? p->sort_skip_bits : bits_used;
-        rc = hcc_sort_range(p->d_keys, n, container, lo, bits_used, perm, p->d_ws, p->ws_bytes, stream);
+        slot = trace_take_slot(bvh);
+        rc = sort_launch(p->d_keys, n, container, lo, bits_used, perm, p->d_ws, p->ws_bytes, s, slot, LK_CHAIN);
         if (rc != HCC_OK) return rc;
     }
-    HCC_CUDA_TRY(cudaEventRecord(p->ev[3], s));
-    rc = hcc_trace(bvh, rays_dev, n, order == HCC_ORDER_NOSORT ? nullptr : perm, mode, hits_dev, stream);
+    if (events) HCC_CUDA_TRY(cudaEventRecord(p->ev[3], s));
+    rc = trace_launch("hcc_reorder_trace", bvh, rays_dev, n, order == HCC_ORDER_NOSORT ? nullptr : perm, mode, hits_dev, nullptr, s,
+                      slot, first);
     if (rc != HCC_OK) return rc;
-    HCC_CUDA_TRY(cudaEventRecord(p->ev[4], s));
-    p->timed = true;
+    if (events) HCC_CUDA_TRY(cudaEventRecord(p->ev[4], s));
+    return HCC_OK;
+}
+
+extern "C" int32_t hcc_reorder_trace(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
+                                     uint32_t key_bits, const float *rays_dev, uint64_t n, int32_t mode,
+                                     void *hits_dev, uint32_t *perm_out_dev, void *stream) {
+    HCC_REQUIRE(p && bvh, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: NULL handle");
+    cudaStream_t s = (cudaStream_t)stream;
+    p->timed = false;
+    int32_t rc = run_chain(p, bvh, cut, order, key_bits, rays_dev, n, mode, hits_dev, perm_out_dev ? perm_out_dev : p->d_perm[0], s,
+                           LK_FIRST, p->timing);
+    if (rc != HCC_OK) return rc;
+    p->timed = p->timing;
     p->timed_host = false;
+    p->last_stream = s;
+    p->calls += 1u;
+    return HCC_OK;
+}
+
+// Both batches of one bounce in one call (PAPER.md:245-247 runs the three kernels per batch; a renderer has the
+// diffuse and the shadow batch of a bounce at the same time).  The second batch's chain starts with a dependent launch
+// that does NOT wait: it is encoded and sorted while the first batch's traversal kernel runs out (its last rays leave
+// most SMs idle), and its own traversal starts as soon as its permutation is complete.  Safe by construction: the second
+// chain's first kernel is launched only after the first batch's trace kernel has passed its own wait, so everything
+// before that trace is complete; the trace reads none of the buffers the second chain writes (keys, sort workspace, the
+// second permutation buffer, its own work counter, its own hits).  The first kernel of the NEXT call on this stream is a
+// plain launch and therefore ordered after both traces.  Both batches must be complete in memory when the call is made.
+extern "C" int32_t hcc_reorder_trace_pair(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order, uint32_t key_bits,
+                                          const float *rays_a_dev, uint64_t n_a, int32_t mode_a, void *hits_a_dev,
+                                          const float *rays_b_dev, uint64_t n_b, int32_t mode_b, void *hits_b_dev, void *stream) {
+    HCC_REQUIRE(p && bvh, HCC_ERR_INVALID_ARG, "hcc_reorder_trace_pair: NULL handle");
+    cudaStream_t s = (cudaStream_t)stream;
+    p->timed = false;
+    int32_t rc = run_chain(p, bvh, cut, order, key_bits, rays_a_dev, n_a, mode_a, hits_a_dev, p->d_perm[0], s, LK_FIRST, false);
+    if (rc != HCC_OK) return rc;
+    rc = run_chain(p, bvh, cut, order, key_bits, rays_b_dev, n_b, mode_b, hits_b_dev, p->d_perm[1], s, n_a ? LK_OVERLAP : LK_FIRST, false);
+    if (rc != HCC_OK) return rc;
+    p->timed_host = false;
+    p->last_stream = s;
+    p->calls += 1u;
     return HCC_OK;
 }
 
@@ -146,20 +196,28 @@ extern "C" int32_t hcc_reorder_trace_host_async(hcc_pipeline *p, const hcc_bvh *
     if (n == 0) return HCC_OK;
     HCC_REQUIRE(rays_host && hits_host, HCC_ERR_INVALID_ARG, "hcc_reorder_trace_host: NULL argument");
     cudaStream_t s = (cudaStream_t)stream;
-    HCC_CUDA_TRY(cudaEventRecord(p->ev[0], s));
+    if (p->timing) HCC_CUDA_TRY(cudaEventRecord(p->ev[0], s));
     HCC_CUDA_TRY(cudaMemcpyAsync(p->d_rays, rays_host, 32 * n, cudaMemcpyHostToDevice, s));
+
     int32_t rc = hcc_reorder_trace(p, bvh, cut, order, key_bits, p->d_rays, n, mode, p->d_hits, nullptr, stream);
     if (rc != HCC_OK) return rc;
     HCC_CUDA_TRY(cudaMemcpyAsync(hits_host, p->d_hits, (mode == HCC_TRACE_CLOSEST ? 16 : 1) * n, cudaMemcpyDeviceToHost, s));
     HCC_CUDA_TRY(cudaEventRecord(p->ev[5], s));
     p->timed_host = true;
+    p->host_pending = true;
     return HCC_OK;
 }
 
 extern "C" int32_t hcc_pipeline_synchronize(hcc_pipeline *p) {
     HCC_REQUIRE(p, HCC_ERR_INVALID_ARG, "hcc_pipeline_synchronize: NULL pipeline");
-    if (!p->timed) return HCC_OK;
-    HCC_CUDA_TRY(cudaEventSynchronize(p->ev[p->timed_host ? 5 : 4]));
+    if (p->host_pending) {
+        HCC_CUDA_TRY(cudaEventSynchronize(p->ev[5]));
+        p->host_pending = false;
+    } else if (p->timed) {
+        HCC_CUDA_TRY(cudaEventSynchronize(p->ev[4]));
+    } else if (p->calls) {
+        HCC_CUDA_TRY(cudaStreamSynchronize(p->last_stream));
+    }
     return HCC_OK;
 }
 
@@ -174,7 +232,7 @@ extern "C" int32_t hcc_reorder_trace_host(hcc_pipeline *p, const hcc_bvh *bvh, c
 
 extern "C" int32_t hcc_pipeline_stage_ms(hcc_pipeline *p, float ms[5]) {
     HCC_REQUIRE(p && ms, HCC_ERR_INVALID_ARG, "hcc_pipeline_stage_ms: NULL argument");
-    HCC_REQUIRE(p->timed, HCC_ERR_INVALID_ARG, "hcc_pipeline_stage_ms: no completed call to time");
+    HCC_REQUIRE(p->timed, HCC_ERR_INVALID_ARG, "hcc_pipeline_stage_ms: no timed call (hcc_pipeline_set_timing first)");
     HCC_CUDA_TRY(cudaEventSynchronize(p->ev[p->timed_host ? 5 : 4]));
     for (int i = 0; i < 3; ++i) HCC_CUDA_TRY(cudaEventElapsedTime(&ms[i], p->ev[1 + i], p->ev[2 + i]));
     ms[3] = ms[4] = 0.0f;

@@ -59,12 +59,24 @@ __device__ __forceinline__ void st_volatile_u32(uint32_t *p, uint32_t v) {
     asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
+// First kernel of a sort: zeroes the control region and the status rows of the passes (uint4 stores) and, for
+// hcc_reorder_trace, the work counter of the trace launch that follows the sort.
+__global__ void __launch_bounds__(256) k_sort_init(uint4 *__restrict__ zero, size_t n_vec, uint32_t *also_zero, int wait) {
+    if (wait) pdl_wait();
+    pdl_trigger();
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_vec; i += stride) zero[i] = make_uint4(0u, 0u, 0u, 0u);
+    if (also_zero && blockIdx.x == 0 && threadIdx.x < 2) also_zero[threadIdx.x] = 0u;
+}
+
 // All digit histograms in one read of the keys.
 template <typename KeyT>
 __global__ void __launch_bounds__(HIST_THREADS)
 k_histogram(const KeyT *__restrict__ keys, uint32_t n, uint32_t passes, uint32_t bit_lo, SortCtl *ctl) {
     __shared__ uint32_t sh[MAX_PASSES][RADIX];
     for (uint32_t i = threadIdx.x; i < MAX_PASSES * RADIX; i += HIST_THREADS) (&sh[0][0])[i] = 0u;
+    pdl_wait();
+    pdl_trigger();
     __syncthreads();
     // 16 bytes of keys per load and HIST_BATCH independent loads in flight per thread: the kernel is
     // a pure stream and would otherwise wait one DRAM round trip per key
@@ -105,6 +117,8 @@ k_scan_hist(SortCtl *ctl, uint32_t *status, size_t status_stride, uint32_t n) {
     __shared__ uint32_t s_w[RADIX / 32];
     __shared__ float s_e[RADIX / 32];
     const uint32_t p = blockIdx.x, d = threadIdx.x, lane = d & 31u, warp = d >> 5;
+    pdl_wait();
+    pdl_trigger();
     uint32_t v = ctl->hist[p][d], incl = v;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -131,6 +145,8 @@ k_scan_hist(SortCtl *ctl, uint32_t *status, size_t status_stride, uint32_t n) {
 
 __global__ void k_iota(uint32_t *perm, uint32_t n) {
     uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    pdl_wait();
+    pdl_trigger();
     if (i < n) perm[i] = i;
 }
 
@@ -155,6 +171,8 @@ k_onesweep(const KeyT *__restrict__ keys_in, KeyT *__restrict__ keys_out, const 
     uint32_t *s_vals = reinterpret_cast<uint32_t *>(s_dyn + sizeof(KeyT) * SORT_TILE);
 
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    pdl_wait();          // the previous pass (or the histogram scan) is complete
+    pdl_trigger();
     const bool use_match = *few_digits != 0u;      // uniform over the grid
     const uint32_t my_base = warp * (SORT_ITEMS * 32) + lane;   // item i at my_base + 32*i (warp-striped)
     KeyT key[SORT_ITEMS];
@@ -317,7 +335,7 @@ static uint64_t ctl_bytes(uint64_t n) {
 }
 
 template <typename KeyT>
-static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t bit_lo, uint32_t *perm, unsigned char *ws, cudaStream_t s) {
+static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t bit_lo, uint32_t *perm, unsigned char *ws, cudaStream_t s, uint32_t *also_zero, LaunchKind kind) {
     const uint32_t tiles = (n + SORT_TILE - 1) / SORT_TILE;
     KeyT *keys_tmp = reinterpret_cast<KeyT *>(ws);
     uint32_t *vals_tmp = reinterpret_cast<uint32_t *>(ws + round_up(sizeof(KeyT) * (uint64_t)n, 256));
@@ -325,12 +343,19 @@ static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t bit_l
     SortCtl *ctl = reinterpret_cast<SortCtl *>(ctl_raw);
     uint32_t *status = reinterpret_cast<uint32_t *>(ctl_raw + round_up(sizeof(SortCtl), 256));
     const size_t status_stride = (size_t)(tiles + 1) * RADIX;
-    HCC_CUDA_TRY(cudaMemsetAsync(ctl_raw, 0, round_up(sizeof(SortCtl), 256) + (size_t)passes * status_stride * sizeof(uint32_t), s));
+    {
+        const size_t zero_bytes = round_up(sizeof(SortCtl), 256) + (size_t)passes * status_stride * sizeof(uint32_t);   // a multiple of 16
+        const size_t n_vec = zero_bytes / 16;
+        size_t blocks = (n_vec + 256 * 8 - 1) / (256 * 8);
+        const size_t cap_init = (size_t)sm_count() * 8;
+        if (blocks > cap_init) blocks = cap_init;
+        HCC_CUDA_TRY(launch_k(kind, k_sort_init, dim3((unsigned)blocks), dim3(256), 0, s, reinterpret_cast<uint4 *>(ctl_raw), n_vec, also_zero, kind_waits(kind)));
+    }
     int hist_blocks = (int)((n + HIST_THREADS * 16 - 1) / (HIST_THREADS * 16));
     int cap = sm_count() * 8;
     if (hist_blocks > cap) hist_blocks = cap;
-    k_histogram<KeyT><<<hist_blocks, HIST_THREADS, 0, s>>>(keys, n, passes, bit_lo, ctl);
-    k_scan_hist<<<passes, RADIX, 0, s>>>(ctl, status, status_stride, n);
+    HCC_CUDA_TRY(launch_k(LK_CHAIN, k_histogram<KeyT>, dim3(hist_blocks), dim3(HIST_THREADS), 0, s, (const KeyT *)keys, n, passes, bit_lo, ctl));
+    HCC_CUDA_TRY(launch_k(LK_CHAIN, k_scan_hist, dim3(passes), dim3(RADIX), 0, s, ctl, status, status_stride, n));
     const size_t dyn = (sizeof(KeyT) + sizeof(uint32_t)) * SORT_TILE;
     constexpr int SORT_THREADS = SortCfg<KeyT>::THREADS;
     // once per device and key width: the dynamic shared-memory limit and the resident CTAs per SM
@@ -357,10 +382,9 @@ static int32_t sort_impl(KeyT *keys, uint32_t n, uint32_t passes, uint32_t bit_l
         uint32_t *tk = &ctl->ticket[p];
         const uint32_t *fd = &ctl->few_digits[p];
         const uint32_t shift = bit_lo + RADIX_BITS * p;
-        if (first && last) k_onesweep<KeyT, true, false><<<grid, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd, tiles);
-        else if (first)    k_onesweep<KeyT, true, true><<<grid, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd, tiles);
-        else if (last)     k_onesweep<KeyT, false, false><<<grid, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd, tiles);
-        else               k_onesweep<KeyT, false, true><<<grid, SORT_THREADS, dyn, s>>>(kin, kout, vin, vout, n, shift, st, tk, fd, tiles);
+        auto kern = first && last ? k_onesweep<KeyT, true, false> : first ? k_onesweep<KeyT, true, true>
+                    : last ? k_onesweep<KeyT, false, false> : k_onesweep<KeyT, false, true>;
+        HCC_CUDA_TRY(launch_k(LK_CHAIN, kern, dim3(grid), dim3(SORT_THREADS), dyn, s, (const KeyT *)kin, kout, (const uint32_t *)vin, vout, n, shift, st, tk, fd, tiles));
         KeyT *t = kin; kin = kout; kout = t;
     }
     HCC_CUDA_TRY(cudaGetLastError());
@@ -379,8 +403,8 @@ extern "C" int32_t hcc_sort_workspace_bytes(uint64_t n, uint32_t container_bits,
     return HCC_OK;
 }
 
-extern "C" int32_t hcc_sort_range(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bit_lo, uint32_t bit_hi,
-                                  uint32_t *perm_dev, void *workspace_dev, uint64_t workspace_bytes, void *stream) {
+int32_t hcc::sort_launch(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bit_lo, uint32_t bit_hi, uint32_t *perm_dev,
+                         void *workspace_dev, uint64_t workspace_bytes, cudaStream_t s, uint32_t *also_zero, LaunchKind kind) {
     HCC_REQUIRE(container_bits == 32 || container_bits == 64, HCC_ERR_INVALID_ARG, "hcc_sort: container_bits must be 32 or 64");
     HCC_REQUIRE(bit_lo <= bit_hi && bit_hi <= container_bits, HCC_ERR_INVALID_ARG, "hcc_sort: need bit_lo <= bit_hi <= container_bits");
     HCC_REQUIRE(n < (1ull << 30), HCC_ERR_UNSUPPORTED, "hcc_sort: n >= 2^30");
@@ -392,16 +416,20 @@ extern "C" int32_t hcc_sort_range(void *keys_dev, uint64_t n, uint32_t container
     hcc_sort_workspace_bytes(n, container_bits, &need);
     HCC_REQUIRE(workspace_bytes >= need, HCC_ERR_INVALID_ARG, "hcc_sort: workspace too small (%llu < %llu)",
                 (unsigned long long)workspace_bytes, (unsigned long long)need);
-    cudaStream_t s = (cudaStream_t)stream;
     const uint32_t passes = (bit_hi - bit_lo + RADIX_BITS - 1) / RADIX_BITS;
+    unsigned char *ws = reinterpret_cast<unsigned char *>(round_up(reinterpret_cast<uintptr_t>(workspace_dev), 256));
     if (passes == 0) {
-        k_iota<<<(uint32_t)((n + 255) / 256), 256, 0, s>>>(perm_dev, (uint32_t)n);
-        HCC_CUDA_TRY(cudaGetLastError());
+        HCC_CUDA_TRY(launch_k(kind, k_sort_init, dim3(1), dim3(256), 0, s, reinterpret_cast<uint4 *>(ws), (size_t)0, also_zero, kind_waits(kind)));
+        HCC_CUDA_TRY(launch_k(LK_CHAIN, k_iota, dim3((uint32_t)((n + 255) / 256)), dim3(256), 0, s, perm_dev, (uint32_t)n));
         return HCC_OK;
     }
-    unsigned char *ws = reinterpret_cast<unsigned char *>(round_up(reinterpret_cast<uintptr_t>(workspace_dev), 256));
-    if (container_bits == 32) return sort_impl<uint32_t>((uint32_t *)keys_dev, (uint32_t)n, passes, bit_lo, perm_dev, ws, s);
-    return sort_impl<unsigned long long>((unsigned long long *)keys_dev, (uint32_t)n, passes, bit_lo, perm_dev, ws, s);
+    if (container_bits == 32) return sort_impl<uint32_t>((uint32_t *)keys_dev, (uint32_t)n, passes, bit_lo, perm_dev, ws, s, also_zero, kind);
+    return sort_impl<unsigned long long>((unsigned long long *)keys_dev, (uint32_t)n, passes, bit_lo, perm_dev, ws, s, also_zero, kind);
+}
+
+extern "C" int32_t hcc_sort_range(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bit_lo, uint32_t bit_hi,
+                                  uint32_t *perm_dev, void *workspace_dev, uint64_t workspace_bytes, void *stream) {
+    return sort_launch(keys_dev, n, container_bits, bit_lo, bit_hi, perm_dev, workspace_dev, workspace_bytes, (cudaStream_t)stream, nullptr, LK_FIRST);
 }
 
 extern "C" int32_t hcc_sort(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bits_used, uint32_t *perm_dev,

@@ -215,6 +215,8 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
 
     if (lane == 0) sts32(sa_tail, 0u);
     __syncwarp();
+    pdl_wait();          // the permutation (or whatever wrote the rays) and the zeroed work counter are complete
+    pdl_trigger();
 #ifdef HCC_TRACE_TIMELINE   // debug builds only: per-warp start / exhaustion / end times behind the eight counters
     unsigned long long tl_t0 = 0, tl_ex = 0;
     if (stats) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tl_t0));
@@ -497,12 +499,27 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
     }
 }
 
+// Zeroes the work counter of the trace launch that follows (a launch that is not preceded by a sort).
+__global__ void k_trace_arm(uint32_t *ctl, int wait) {
+    if (wait) pdl_wait();
+    pdl_trigger();
+    if (threadIdx.x < 2) ctl[threadIdx.x] = 0u;
+}
+
 }  // namespace hcc
 
 using namespace hcc;
 
-static int32_t trace_impl(const char *who, const hcc_bvh *bvh, const float *rays_dev, uint64_t n, const uint32_t *perm_dev,
-                          int32_t mode, void *hits_dev, unsigned long long *stats_dev, void *stream) {
+// every launch takes the next counter slot of the ring, so launches in flight on different streams never share a
+// counter (up to HCC_TRACE_SLOTS of them); the slot is zeroed on the launch stream by a kernel before the trace
+// kernel (the sort's first kernel or k_trace_arm), so an aborted launch leaves nothing behind
+uint32_t *hcc::trace_take_slot(const hcc_bvh *bvh) {
+    return bvh->d_trace_ctl + 2u * (bvh->trace_calls->fetch_add(1u) % (uint32_t)HCC_TRACE_SLOTS);
+}
+
+int32_t hcc::trace_launch(const char *who, const hcc_bvh *bvh, const float *rays_dev, uint64_t n, const uint32_t *perm_dev,
+                          int32_t mode, void *hits_dev, unsigned long long *stats_dev, cudaStream_t s, uint32_t *armed_slot,
+                          LaunchKind kind) {
     HCC_REQUIRE(bvh, HCC_ERR_INVALID_ARG, "%s: NULL bvh", who);
     HCC_REQUIRE(mode == HCC_TRACE_CLOSEST || mode == HCC_TRACE_ANY, HCC_ERR_INVALID_ARG, "%s: unknown mode %d", who, mode);
     if (n == 0) return HCC_OK;
@@ -511,44 +528,36 @@ static int32_t trace_impl(const char *who, const hcc_bvh *bvh, const float *rays
                 "%s: rays need 32-byte, hits and perm 16-byte alignment", who);
     // the rank counter runs up to n + 32 * (warps of the grid) before every warp has seen it exhausted
     HCC_REQUIRE(n < (1ull << 32) - (1ull << 24), HCC_ERR_UNSUPPORTED, "%s: n >= 2^32 - 2^24", who);
-    cudaStream_t s = (cudaStream_t)stream;
     const uint32_t cap = (uint32_t)sm_count() * (mode == HCC_TRACE_ANY ? TRACE_BLOCKS_PER_SM_ANY : TRACE_BLOCKS_PER_SM);
     const uint32_t want = (uint32_t)((n + TRACE_THREADS - 1) / TRACE_THREADS);
     const uint32_t blocks = want < cap ? want : cap;
     TraceScene sc;
     sc.wrec = bvh->d_wrec; sc.ttri = bvh->d_ttri; sc.root_ref = bvh->root_ref;
     for (int a = 0; a < 3; ++a) { sc.q_lo[a] = bvh->q_lo[a]; sc.q_scale[a] = bvh->q_scale[a]; }
-    // every launch takes the next counter slot of the ring and zeroes it on its own stream first, so
-    // launches in flight on different streams never share a counter (up to HCC_TRACE_SLOTS of them)
-    // and an aborted launch leaves nothing behind
-    uint32_t *ctl = bvh->d_trace_ctl + 2u * (bvh->trace_calls->fetch_add(1u) % (uint32_t)HCC_TRACE_SLOTS);
-    HCC_CUDA_TRY(cudaMemsetAsync(ctl, 0, 2 * sizeof(uint32_t), s));
-    const float4 *rays = (const float4 *)rays_dev;
-#ifdef HCC_TRACE_TIMELINE
-    if (stats_dev) {
-        if (mode == HCC_TRACE_CLOSEST) k_trace<false, false><<<blocks, TRACE_THREADS, 0, s>>>(sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, stats_dev);
-        else                           k_trace<true, false><<<blocks, TRACE_THREADS, 0, s>>>(sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, stats_dev);
-    } else
-#endif
-    if (stats_dev) {
-        if (mode == HCC_TRACE_CLOSEST) k_trace<false, true><<<blocks, TRACE_THREADS, 0, s>>>(sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, stats_dev);
-        else                           k_trace<true, true><<<blocks, TRACE_THREADS, 0, s>>>(sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, stats_dev);
-    } else {
-        if (mode == HCC_TRACE_CLOSEST) k_trace<false, false><<<blocks, TRACE_THREADS, 0, s>>>(sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, nullptr);
-        else                           k_trace<true, false><<<blocks, TRACE_THREADS, 0, s>>>(sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, nullptr);
+    uint32_t *ctl = armed_slot;
+    if (!ctl) {
+        ctl = trace_take_slot(bvh);
+        HCC_CUDA_TRY(launch_k(kind, k_trace_arm, dim3(1), dim3(32), 0, s, ctl, kind_waits(kind)));
     }
-    HCC_CUDA_TRY(cudaGetLastError());
+    const float4 *rays = (const float4 *)rays_dev;
+    const bool any = mode == HCC_TRACE_ANY;
+#ifdef HCC_TRACE_TIMELINE   // debug builds: the plain kernel writes its per-warp times behind the counters
+    auto kern = any ? k_trace<true, false> : k_trace<false, false>;
+#else
+    auto kern = stats_dev ? (any ? k_trace<true, true> : k_trace<false, true>) : (any ? k_trace<true, false> : k_trace<false, false>);
+#endif
+    HCC_CUDA_TRY(launch_k(LK_CHAIN, kern, dim3(blocks), dim3(TRACE_THREADS), 0, s, sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, stats_dev));
     return HCC_OK;
 }
 
 extern "C" int32_t hcc_trace(const hcc_bvh *bvh, const float *rays_dev, uint64_t n, const uint32_t *perm_dev,
                              int32_t mode, void *hits_dev, void *stream) {
-    return trace_impl("hcc_trace", bvh, rays_dev, n, perm_dev, mode, hits_dev, nullptr, stream);
+    return trace_launch("hcc_trace", bvh, rays_dev, n, perm_dev, mode, hits_dev, nullptr, (cudaStream_t)stream, nullptr, LK_FIRST);
 }
 
 extern "C" int32_t hcc_trace_stats(const hcc_bvh *bvh, const float *rays_dev, uint64_t n, const uint32_t *perm_dev,
                                    int32_t mode, void *hits_dev, uint64_t *stats_dev, void *stream) {
     HCC_REQUIRE(stats_dev && aligned(stats_dev, 16), HCC_ERR_INVALID_ARG, "hcc_trace_stats: stats_dev NULL or misaligned");
     HCC_CUDA_TRY(cudaMemsetAsync(stats_dev, 0, 8 * sizeof(uint64_t), (cudaStream_t)stream));
-    return trace_impl("hcc_trace_stats", bvh, rays_dev, n, perm_dev, mode, hits_dev, (unsigned long long *)stats_dev, stream);
+    return trace_launch("hcc_trace_stats", bvh, rays_dev, n, perm_dev, mode, hits_dev, (unsigned long long *)stats_dev, (cudaStream_t)stream, nullptr, LK_FIRST);
 }

@@ -148,6 +148,7 @@ def test_reorder_trace_host_async_matches_the_device_path(hcc, cases):
     hits_a = torch.empty((n_d, 4), dtype=torch.float32).pin_memory()
     hits_b = torch.empty(n_s, dtype=torch.uint8).pin_memory()
     torch.cuda.synchronize()
+    pa.set_timing(True)
     for _ in range(3):
         hits_a.zero_(); hits_b.zero_()
         pa.reorder_trace_host_async(d["bvh"], cut, hcc.ORDER_HCC, rays_a, hits_a, hcc.TRACE_CLOSEST, stream=sa)

@@ -326,6 +326,9 @@ def test_pipeline_matches_stages(hcc, dev_cases, name, K, bits):
     cut = hcc.select_cut(d["bvh"], hcc.density(d["bvh"]), K, bits)
     n_max = max(d["diffuse"].shape[0], d["shadow"].shape[0])
     pipe = hcc.Pipeline(n_max, 64, host_staging=True)
+    with pytest.raises(hcc.HccError):
+        pipe.stage_ms()                       # nothing timed yet
+    pipe.set_timing(True)
     for batch, mode in (("diffuse", hcc.TRACE_CLOSEST), ("shadow", hcc.TRACE_ANY)):
         ref = hcc.trace(d["bvh"], d[batch], None, mode)
         for order in (hcc.ORDER_NOSORT, hcc.ORDER_TWOPOINT, hcc.ORDER_HCC):
@@ -343,6 +346,38 @@ def test_pipeline_matches_stages(hcc, dev_cases, name, K, bits):
             hits_h = torch.empty(ref.shape, dtype=ref.dtype).pin_memory()
             pipe.reorder_trace_host(d["bvh"], cut, order, rays_h, hits_h, mode, key_bits=bits)
             assert torch.equal(hits_h.view(torch.uint8), ref.cpu().view(torch.uint8))
+    pipe.close()
+
+
+@pytest.mark.parametrize("name,K,bits", [("tiny", 64, 32), ("room_mid", 1024, 32), ("room_mid", 4096, 64)])
+def test_pipeline_pair_matches_two_calls(hcc, dev_cases, name, K, bits):
+    """hcc_reorder_trace_pair (batch b's chain overlaps batch a's traversal by dependent launch) gives the hits of the
+    separate calls, for the three orders, repeatedly (the chains of successive pairs reuse the pipeline's buffers), with
+    an empty first or second batch, and with HCC_NO_PDL-style plain launches covered by the single-call tests."""
+    d = dev_cases[name]
+    cut = hcc.select_cut(d["bvh"], hcc.density(d["bvh"]), K, bits)
+    ra, rb = d["diffuse"], d["shadow"]
+    pipe = hcc.Pipeline(max(ra.shape[0], rb.shape[0]), 64)
+    ref_a = hcc.trace(d["bvh"], ra, None, hcc.TRACE_CLOSEST)
+    ref_b = hcc.trace(d["bvh"], rb, None, hcc.TRACE_ANY)
+    ha, hb = torch.empty_like(ref_a), torch.empty_like(ref_b)
+    for rep in range(4):
+        for order in (hcc.ORDER_HCC, hcc.ORDER_NOSORT, hcc.ORDER_TWOPOINT):
+            ha.fill_(-1.0); hb.fill_(7)
+            pipe.reorder_trace_pair(d["bvh"], cut, order, ra, hcc.TRACE_CLOSEST, ha, rb, hcc.TRACE_ANY, hb, key_bits=bits)
+            assert torch.equal(ha.view(torch.int32), ref_a.view(torch.int32)) and torch.equal(hb, ref_b), (rep, order)
+    # the batches the other way round, and one of them empty
+    ha.fill_(-1.0); hb.fill_(7)
+    pipe.reorder_trace_pair(d["bvh"], cut, hcc.ORDER_HCC, rb, hcc.TRACE_ANY, hb, ra, hcc.TRACE_CLOSEST, ha, key_bits=bits)
+    assert torch.equal(ha.view(torch.int32), ref_a.view(torch.int32)) and torch.equal(hb, ref_b)
+    empty = ra[:0]
+    he = torch.empty((0, 4), dtype=torch.float32, device="cuda")
+    hb.fill_(7)
+    pipe.reorder_trace_pair(d["bvh"], cut, hcc.ORDER_HCC, empty, hcc.TRACE_CLOSEST, he, rb, hcc.TRACE_ANY, hb, key_bits=bits)
+    assert torch.equal(hb, ref_b)
+    ha.fill_(-1.0)
+    pipe.reorder_trace_pair(d["bvh"], cut, hcc.ORDER_HCC, ra, hcc.TRACE_CLOSEST, ha, rb[:0], hcc.TRACE_ANY, hb[:0], key_bits=bits)
+    assert torch.equal(ha.view(torch.int32), ref_a.view(torch.int32))
     pipe.close()
 
 
