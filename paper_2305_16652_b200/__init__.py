@@ -140,8 +140,8 @@ class Bvh:
         self.scene_hi = np.array(list(hi), dtype=np.float32)
 
     def close(self):
-        if getattr(self, "_h", None) is not None and self._h:
-            lib().hcc_bvh_destroy(self._h)
+        if getattr(self, "_h", None) is not None and self._h and _lib is not None:   # _lib is None at interpreter exit
+            _lib.hcc_bvh_destroy(self._h)
             self._h = None
 
     __del__ = close
@@ -193,8 +193,8 @@ class Cut:
         return boxes
 
     def close(self):
-        if getattr(self, "_h", None) is not None and self._h:
-            lib().hcc_cut_destroy(self._h)
+        if getattr(self, "_h", None) is not None and self._h and _lib is not None:   # _lib is None at interpreter exit
+            _lib.hcc_cut_destroy(self._h)
             self._h = None
 
     __del__ = close
@@ -438,8 +438,8 @@ class Pipeline:
         return dict(encode=ms[0], sort=ms[1], trace=ms[2], h2d=ms[3], d2h=ms[4])
 
     def close(self):
-        if getattr(self, "_h", None) is not None and self._h:
-            lib().hcc_pipeline_destroy(self._h)
+        if getattr(self, "_h", None) is not None and self._h and _lib is not None:   # _lib is None at interpreter exit
+            _lib.hcc_pipeline_destroy(self._h)
             self._h = None
 
     __del__ = close

@@ -85,13 +85,21 @@ __device__ __forceinline__ uint32_t table_mask(const RayEnc &r, const ulonglong2
 }
 
 constexpr int ENC_THREADS = 256;
-constexpr int ENC_THREADS_MAX = 1024;   // one big CTA per SM when the staged tables leave room for only one
+// The HCC encoder's CTA shapes: its speed is set by how many warps an SM holds (the slab tests are chains of
+// dependent fp32 operations on the half-rate min/max pipe), so the staged tables are shared by as many threads as
+// possible: two CTAs of 768 threads at <= 40 registers (48 warps per SM) while two copies of the tables fit, else one
+// CTA of 1024 threads.
+#ifndef HCC_ENC_WIDE_THREADS
+#define HCC_ENC_WIDE_THREADS 768
+#define HCC_ENC_WIDE_CTAS 2
+#endif
+constexpr int ENC_WIDE_THREADS = HCC_ENC_WIDE_THREADS, ENC_WIDE_CTAS = HCC_ENC_WIDE_CTAS, ENC_MAX_THREADS = 1024;
 
 // Alg. 1: line 1 "copy cut nodes from global memory into shared memory" (the first
 // smem_entries entries = whole levels), line 2 grid-stride "while have ray", lines 4-6 per
 // level.  One ray per thread per iteration; 32-byte rays read as two 16-byte loads.
-template <typename KeyT>
-__global__ void __launch_bounds__(ENC_THREADS_MAX)
+template <typename KeyT, int THREADS, int MIN_CTAS>
+__global__ void __launch_bounds__(THREADS, MIN_CTAS)
 k_encode_hcc(const float4 *__restrict__ rays, uint64_t n, const CutDev cut, uint32_t smem_entries,
              KeyT *__restrict__ keys, int wait) {
     extern __shared__ ulonglong2 s_box[];
@@ -145,18 +153,30 @@ __device__ __forceinline__ uint32_t quantise(float p, float lo, float hi, float 
     return (uint32_t)x;
 }
 
+// spread5[x]: bit i of the 5-bit x at bit 6 * i (the Morton stride of six interleaved coordinates)
+__device__ __forceinline__ uint32_t spread5_of(uint32_t x) {
+    return (x & 1u) | ((x & 2u) << 5) | ((x & 4u) << 10) | ((x & 8u) << 15) | ((x & 16u) << 20);
+}
+
 template <typename KeyT>
 __global__ void __launch_bounds__(ENC_THREADS)
 k_encode_twopoint(const float4 *__restrict__ rays, uint64_t n, float3 lo, float3 hi, float len, uint32_t b,
                   KeyT *__restrict__ keys, int wait) {
+    // the interleave as table look-ups: 32 words, one per bank, so any mix of indices in a warp is conflict-free
+    __shared__ uint32_t s_spread[32];
+    if (threadIdx.x < 32) s_spread[threadIdx.x] = spread5_of(threadIdx.x);
     if (wait) pdl_wait();
     pdl_trigger();
+    __syncthreads();
     const uint64_t stride = (uint64_t)gridDim.x * ENC_THREADS;
     const float scale = (float)(1u << b);
     const uint32_t qmax = (1u << b) - 1u;
-    for (uint64_t ri = (uint64_t)blockIdx.x * ENC_THREADS + threadIdx.x; ri < n; ri += stride) {
-        float4 o, d;
-        ld_ray(rays + 2 * ri, o, d);
+    uint64_t ri = (uint64_t)blockIdx.x * ENC_THREADS + threadIdx.x;
+    float4 no = make_float4(0.f, 0.f, 0.f, 0.f), nd = no;
+    if (ri < n) ld_ray(rays + 2 * ri, no, nd);
+    for (; ri < n; ri += stride) {
+        const float4 o = no, d = nd;
+        if (ri + stride < n) ld_ray(rays + 2 * (ri + stride), no, nd);     // the next ray arrives while this one is coded
         uint32_t q[6];
         q[0] = quantise(o.x, lo.x, hi.x, scale, qmax);
         q[1] = quantise(o.y, lo.y, hi.y, scale, qmax);
@@ -164,10 +184,13 @@ k_encode_twopoint(const float4 *__restrict__ rays, uint64_t n, float3 lo, float3
         q[3] = quantise(o.x + len * d.x, lo.x, hi.x, scale, qmax);
         q[4] = quantise(o.y + len * d.y, lo.y, hi.y, scale, qmax);
         q[5] = quantise(o.z + len * d.z, lo.z, hi.z, scale, qmax);
+        // coordinate c's bit i sits at key bit 6 * i + (5 - c): o.x first from the top (R10); b <= 10
         unsigned long long key = 0;
-        for (int i = (int)b - 1; i >= 0; --i) {
 #pragma unroll
-            for (int c = 0; c < 6; ++c) key = (key << 1) | ((q[c] >> i) & 1u);
+        for (int c = 0; c < 6; ++c) {
+            unsigned long long s_ = s_spread[q[c] & 31u];
+            if (sizeof(KeyT) == 8) s_ |= (unsigned long long)s_spread[(q[c] >> 5) & 31u] << 30;
+            key |= s_ << (5 - c);
         }
         keys[ri] = (KeyT)key;
     }
@@ -247,7 +270,8 @@ static cudaError_t encode_attr(size_t budget) {
     static std::atomic<int> done[HCC_MAX_DEVICES];
     const int dev = current_device();
     if (done[dev].load(std::memory_order_acquire)) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(k_encode_hcc<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget);
+    cudaError_t e = cudaFuncSetAttribute(k_encode_hcc<KeyT, ENC_WIDE_THREADS, ENC_WIDE_CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_encode_hcc<KeyT, ENC_MAX_THREADS, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget);
     if (e == cudaSuccess) done[dev].store(1, std::memory_order_release);
     return e;
 }
@@ -272,18 +296,29 @@ int32_t hcc::encode_launch(const float *rays_dev, uint64_t n, const hcc_cut *cut
         if ((size_t)end * 32 <= budget) smem_entries = end; else break;
     }
     size_t smem = (size_t)smem_entries * 32;
-    // CTA size: as many resident threads per SM as the staged tables allow
-    const int threads = smem > 100 * 1024 ? 1024 : smem > 48 * 1024 ? 512 : ENC_THREADS;
+    const bool wide = ENC_WIDE_CTAS * (smem + 1024) <= 200 * 1024;     // two CTAs' tables (+ the per-CTA reserve) fit one SM
     if (cut->container_bits == 32) {
-        auto kern = k_encode_hcc<uint32_t>;
         HCC_CUDA_TRY(encode_attr<uint32_t>(budget));
-        HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, smem, n, threads)), dim3(threads), smem, s,
-                                (const float4 *)rays_dev, n, d, smem_entries, (uint32_t *)keys_dev, kind_waits(kind)));
+        if (wide) {
+            auto kern = k_encode_hcc<uint32_t, ENC_WIDE_THREADS, ENC_WIDE_CTAS>;
+            HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, smem, n, ENC_WIDE_THREADS)), dim3(ENC_WIDE_THREADS), smem, s,
+                                  (const float4 *)rays_dev, n, d, smem_entries, (uint32_t *)keys_dev, kind_waits(kind)));
+        } else {
+            auto kern = k_encode_hcc<uint32_t, ENC_MAX_THREADS, 1>;
+            HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, smem, n, ENC_MAX_THREADS)), dim3(ENC_MAX_THREADS), smem, s,
+                                  (const float4 *)rays_dev, n, d, smem_entries, (uint32_t *)keys_dev, kind_waits(kind)));
+        }
     } else {
-        auto kern = k_encode_hcc<unsigned long long>;
         HCC_CUDA_TRY(encode_attr<unsigned long long>(budget));
-        HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, smem, n, threads)), dim3(threads), smem, s,
-                                (const float4 *)rays_dev, n, d, smem_entries, (unsigned long long *)keys_dev, kind_waits(kind)));
+        if (wide) {
+            auto kern = k_encode_hcc<unsigned long long, ENC_WIDE_THREADS, ENC_WIDE_CTAS>;
+            HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, smem, n, ENC_WIDE_THREADS)), dim3(ENC_WIDE_THREADS), smem, s,
+                                  (const float4 *)rays_dev, n, d, smem_entries, (unsigned long long *)keys_dev, kind_waits(kind)));
+        } else {
+            auto kern = k_encode_hcc<unsigned long long, ENC_MAX_THREADS, 1>;
+            HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, smem, n, ENC_MAX_THREADS)), dim3(ENC_MAX_THREADS), smem, s,
+                                  (const float4 *)rays_dev, n, d, smem_entries, (unsigned long long *)keys_dev, kind_waits(kind)));
+        }
     }
     return HCC_OK;
 }
