@@ -368,7 +368,9 @@ def run_ours(args):
         orders = {}
         for name, order in ORDERS:
             ms, stage, _ = timed(sc, order, k, 3, per_stage=True)
-            o = {"ms_per_step": ms, "mrays_per_s_incl": sc.n / ms / 1e3}
+            ms_pair, _, _ = timed(sc, order, k, 3)       # the same step as ONE hcc_reorder_trace_pair call (chained launches)
+            o = {"ms_per_step": ms, "mrays_per_s_incl": sc.n / ms / 1e3, "pair_ms_per_step": ms_pair,
+                 "pair_mrays_per_s_incl": sc.n / ms_pair / 1e3}
             for bn, nb in (("diffuse", sc.n_d), ("shadow", sc.n_s)):
                 st = stage[bn]
                 tot = st["encode"] + st["sort"] + st["trace"]
@@ -384,6 +386,8 @@ def run_ours(args):
                          "trace_vs_twopoint": h["mrays_per_s_trace_only"] / orders["twopoint"][bn]["mrays_per_s_trace_only"]}
         speed["all_incl_vs_nosort"] = orders["nosort"]["ms_per_step"] / orders["hcc"]["ms_per_step"]
         speed["all_incl_vs_twopoint"] = orders["twopoint"]["ms_per_step"] / orders["hcc"]["ms_per_step"]
+        speed["pair_incl_vs_nosort"] = orders["nosort"]["pair_ms_per_step"] / orders["hcc"]["pair_ms_per_step"]
+        speed["pair_incl_vs_twopoint"] = orders["twopoint"]["pair_ms_per_step"] / orders["hcc"]["pair_ms_per_step"]
         return orders, speed
 
     def order_perms(sc, rays):
@@ -406,7 +410,7 @@ def run_ours(args):
                 st = hcc.trace_stats(sc.bvh, rays, pm, mode)
                 o[on] = {"node_records_per_ray": st["nodes"] / max(st["rays"], 1), "tri_tests_per_ray": st["tris"] / max(st["rays"], 1),
                          "distinct_records_per_warp_step": st["records_per_step"], "lanes_per_warp_step": st["lanes_per_step"],
-                         "lanes_per_tri_round": st["lanes_per_tri_round"], "max_stack": st["max_stack"],
+                         "tri_tests_per_round": st["tri_tests_per_round"], "max_stack": st["max_stack"],
                          "lane_ops": st["nodes"] * OPS_NODE + st["tris"] * OPS_TRI}
             out[name] = {"anc_hcc": hcc.anc(keys0, perms["hcc"]), "anc_nosort": hcc.anc(keys0, None), "orders": o}
         return out

@@ -99,10 +99,12 @@ HCC_API int32_t hcc_version(void);
  * adjacent, parent < child, every node reachable once, leaf count in 1..8, depth <= 63,
  * fewer than 2^27 triangles and 2^30 nodes:
  * otherwise HCC_ERR_INVALID_ARG / HCC_ERR_UNSUPPORTED), copies them to the device and runs
- * the conversion kernels on `stream`: one 32-byte traversal record per internal node
- * (both child boxes as 15-bit cells of a uniform grid over the root box, rounded outwards
- * and padded by one cell, plus the two child references), the 64-byte triangle records in
- * leaf order, parent links and sub-tree leaf counts.  The quantised boxes only cull: results
+ * the conversion kernels on `stream`: the binary tree is collapsed on the host into a 4-wide
+ * traversal tree (the internal child with the largest surface area is opened until a node has
+ * four children) with one 64-byte record per wide node (four child boxes as 15-bit cells of a
+ * uniform grid over the root box, rounded outwards and padded by one cell, plus the four child
+ * references; a leaf of 5..8 triangles becomes two leaves under a wide node of its own), the
+ * 64-byte triangle records in leaf order, parent links and sub-tree leaf counts.  The quantised boxes only cull: results
  * are defined by the triangle predicate under hcc_trace.  All three arrays are host pointers, read before return.
  * The call synchronises `stream` before returning. */
 HCC_API int32_t hcc_bvh_create(const hcc_node *nodes_host, uint32_t n_nodes, const float *tris_host,
@@ -245,11 +247,15 @@ HCC_API int32_t hcc_sort_range(void *keys_dev, uint64_t n, uint32_t container_bi
                        uint32_t *perm_dev, void *workspace_dev, uint64_t workspace_bytes, void *stream);
 
 /* ---- (a4) trace -----------------------------------------------------------------------
- * Rays are traced in the order perm_dev[0], perm_dev[1], ... (perm_dev == NULL: 0, 1, ...,
- * the NoSort order): warps take consecutive 32-rank chunks of that order, and every result
- * is written at the ray's own index ("the trace kernel fetches the rays based
- * on these sorted indices").  n < 2^32 - 2^24.  Up to 1024 trace launches on one hcc_bvh may
- * be in flight at a time (each takes its own work counter, zeroed on `stream`).  The quantised
+ * Rays are traced through perm_dev (perm_dev == NULL: the input order 0, 1, ..., the NoSort
+ * order): warps take 32-rank chunks of consecutive ranks, so the rays a warp holds are
+ * neighbours in the given order, and every result is written at the ray's own index
+ * ("the trace kernel fetches the rays based on these sorted indices").  The chunks
+ * of a permutation are handed out from its END (descending keys: hierarchy cut codes carry the
+ * densest cut nodes in their top bits, so the rays with the most traversal work start first and
+ * the kernel runs out on cheap ones); which warp traces which chunk when has no effect on any
+ * result.  n < 2^32 - 2^24.  Up to 1024 trace launches on one hcc_bvh may be in flight at a
+ * time (each takes its own work counter, zeroed on `stream` by a kernel of the call).  The quantised
  * boxes are tested with a slack proportional to the distance of the ray origin from the scene
  * (2^-20 of it), which covers the fp32 rounding of the plane distances for origins up to about
  * 10^4 scene extents away; beyond that a triangle may be culled that the predicate would accept.  CLOSEST: hits_dev = hcc_hit[n]: the triangle with the
@@ -262,12 +268,13 @@ HCC_API int32_t hcc_trace(const hcc_bvh *bvh, const float *rays_dev, uint64_t n,
                   int32_t mode, void *hits_dev, void *stream);
 
 /* Same traversal, instrumented (never used for timing): stats_dev = uint64[8], zeroed by the
- * call, then [0] = sibling-pair records fetched by rays (32 bytes each), [1] = triangle records
+ * call, then [0] = wide-node records fetched by rays (64 bytes each), [1] = triangle records
  * fetched (64 bytes each), [2] = rays traced, [3] = deepest traversal stack, and per WARP-level
  * node step (the 32 rays a warp holds fetch their records with one load instruction): [4] =
  * distinct records fetched, summed over steps, [5] = steps, [6] = lanes taking part, summed.
  * [4]/[5] is what a coherent order lowers (rays of a warp sharing node
- * fetches); [0] does not depend on the order.  [7] is reserved.  hits_dev as hcc_trace. */
+ * fetches); [0] hardly depends on the order.  [7] = warp-level triangle rounds ([1]/[7] =
+ * triangle tests per round).  hits_dev as hcc_trace. */
 HCC_API int32_t hcc_trace_stats(const hcc_bvh *bvh, const float *rays_dev, uint64_t n, const uint32_t *perm_dev,
                         int32_t mode, void *hits_dev, uint64_t *stats_dev, void *stream);
 

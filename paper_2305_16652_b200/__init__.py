@@ -352,7 +352,7 @@ def trace_stats(bvh, rays, perm=None, mode=TRACE_CLOSEST, stream=None):
                 node_bytes_per_ray=64.0 * nodes / max(nr, 1), tri_bytes_per_ray=64.0 * tris / max(nr, 1),
                 warp_steps=steps, records_per_step=records / max(steps, 1), lanes_per_step=lanes / max(steps, 1),
                 distinct_node_bytes_per_ray=64.0 * records / max(nr, 1),
-                tri_rounds=rounds, lanes_per_tri_round=tris / max(rounds, 1))
+                tri_rounds=rounds, tri_tests_per_round=tris / max(rounds, 1), lanes_per_tri_round=tris / max(rounds, 1))
 
 
 def anc(keys, perm=None, stream=None):
