@@ -314,11 +314,12 @@ HCC_API int32_t hcc_reorder_trace_host_async(hcc_pipeline *p, const hcc_bvh *bvh
                                      uint32_t key_bits, const float *rays_host, uint64_t n, int32_t mode,
                                      void *hits_host, void *stream);
 /* Both batches of one bounce in one call: batch a (say the diffuse rays, HCC_TRACE_CLOSEST) and batch b (the
- * shadow rays, HCC_TRACE_ANY) go through the same three kernels as in hcc_reorder_trace, a first.  The kernels
- * are chained by programmatic dependent launch and batch b's chain starts WITHOUT waiting for batch a's trace
- * kernel: b is encoded and sorted while a's traversal runs out, so both batches must be complete in memory
- * when the call is made (no kernel enqueued in between can have produced b's rays: there is none).  Results
- * are those of two hcc_reorder_trace calls.  Either n may be 0.  Per-stage timing is not recorded. */
+ * shadow rays, HCC_TRACE_ANY) go through the same three kernels as in hcc_reorder_trace, scheduled so that they
+ * fill each other's gaps: b's keys and sort run on a stream of the pipeline's own beside a's (forked from and
+ * joined back into `stream` by events), then a's traversal kernel and, as a dependent launch that does not wait
+ * for it, b's: b's CTAs become resident as a's run out.  Both batches must be complete in memory when the call
+ * is made.  Results are those of two hcc_reorder_trace calls.  Either n may be 0.  The first call allocates a
+ * second key buffer and sort workspace.  Per-stage timing is not recorded. */
 HCC_API int32_t hcc_reorder_trace_pair(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
                                uint32_t key_bits, const float *rays_a_dev, uint64_t n_a, int32_t mode_a,
                                void *hits_a_dev, const float *rays_b_dev, uint64_t n_b, int32_t mode_b,

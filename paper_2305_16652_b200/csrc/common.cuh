@@ -162,8 +162,9 @@ int32_t encode_twopoint_launch(const float *rays_dev, uint64_t n, const float sc
 int32_t sort_launch(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bit_lo, uint32_t bit_hi, uint32_t *perm_dev,
                     void *workspace_dev, uint64_t workspace_bytes, cudaStream_t s, uint32_t *also_zero, LaunchKind kind);
 uint32_t *trace_take_slot(const hcc_bvh *bvh);
-// armed_slot: a work counter already zeroed by a kernel earlier in the chain (the trace kernel is then a chained
-// launch), or NULL (then a one-warp kernel launched as `kind` zeroes a fresh one first)
+int32_t trace_arm(uint32_t *slot, cudaStream_t s);      // zero a work counter by a plain one-warp launch
+// armed_slot: a work counter already zeroed by an earlier kernel: the trace kernel itself is launched as `kind`; or
+// NULL: a one-warp kernel launched as `kind` zeroes a fresh counter and the trace kernel is a chained launch behind it
 int32_t trace_launch(const char *who, const hcc_bvh *bvh, const float *rays_dev, uint64_t n, const uint32_t *perm_dev, int32_t mode,
                      void *hits_dev, unsigned long long *stats_dev, cudaStream_t s, uint32_t *armed_slot, LaunchKind kind);
 }

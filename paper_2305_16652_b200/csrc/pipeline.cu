@@ -18,6 +18,10 @@ struct hcc_pipeline {
     bool timing;           // record the per-stage events (hcc_pipeline_set_timing)
     void *d_ws;
     uint64_t ws_bytes;
+    // hcc_reorder_trace_pair: the second batch's keys and sort run on a stream of the pipeline's own, in scratch of their own
+    void *d_keys2, *d_ws2;
+    cudaStream_t side;
+    cudaEvent_t ev_fork, ev_join;
     float *d_rays;      // host-buffer form only
     void *d_hits;       // host-buffer form only
     cudaEvent_t ev[6];  // h2d start, encode start, sort start, trace start, trace end, d2h end
@@ -56,6 +60,11 @@ extern "C" int32_t hcc_pipeline_destroy(hcc_pipeline *p) {
     cudaFree(p->d_perm[0]);
     cudaFree(p->d_perm[1]);
     cudaFree(p->d_ws);
+    cudaFree(p->d_keys2);
+    cudaFree(p->d_ws2);
+    if (p->side) cudaStreamDestroy(p->side);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
     cudaFree(p->d_rays);
     cudaFree(p->d_hits);
     for (int i = 0; i < 6; ++i)
@@ -107,43 +116,52 @@ extern "C" int32_t hcc_pipeline_set_timing(hcc_pipeline *p, uint32_t enable) {
     return HCC_OK;
 }
 
-// One batch: key kernel -> sort kernels -> trace kernel as one chain of dependent launches (common.cuh).  `first` is how
-// the chain's first kernel is launched; `events` records the per-stage events between the stages.
-static int32_t run_chain(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order, uint32_t key_bits,
-                         const float *rays_dev, uint64_t n, int32_t mode, void *hits_dev, uint32_t *perm, cudaStream_t s,
-                         LaunchKind first, bool events) {
+struct BatchPlan {
+    uint32_t container, bits_used;
+};
+
+static int32_t plan_batch(const hcc_pipeline *p, const hcc_cut *cut, int32_t order, uint32_t key_bits, uint64_t n, int32_t mode,
+                          BatchPlan *out) {
     HCC_REQUIRE(order == HCC_ORDER_NOSORT || order == HCC_ORDER_TWOPOINT || order == HCC_ORDER_HCC, HCC_ERR_INVALID_ARG,
                 "hcc_reorder_trace: unknown order %d", order);
     HCC_REQUIRE(n <= p->n_max, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: n exceeds the pipeline's n_max");
     HCC_REQUIRE(mode == HCC_TRACE_CLOSEST || mode == HCC_TRACE_ANY, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: unknown mode %d", mode);
-    uint32_t container = 32, bits_used = 0;
+    out->container = 32; out->bits_used = 0;
     if (order == HCC_ORDER_HCC) {
         HCC_REQUIRE(cut && cut->valid, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: order HCC needs a selected cut");
-        container = cut->container_bits;
-        bits_used = cut->dev.bits_used;
+        out->container = cut->container_bits;
+        out->bits_used = cut->dev.bits_used;
     } else if (order == HCC_ORDER_TWOPOINT) {
-        container = key_bits <= 32 ? 32u : 64u;
-        bits_used = 6u * (key_bits / 6u);
+        out->container = key_bits <= 32 ? 32u : 64u;
+        out->bits_used = 6u * (key_bits / 6u);
     }
-    HCC_REQUIRE(container <= p->container_bits_max, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: 64-bit keys in a 32-bit pipeline");
+    HCC_REQUIRE(out->container <= p->container_bits_max, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: 64-bit keys in a 32-bit pipeline");
+    return HCC_OK;
+}
+
+// Key kernel -> sort kernels of one batch on stream s, as a chain of dependent launches whose first kernel is a plain
+// launch; *slot receives the batch's trace work counter, zeroed by a kernel of this chain.  `events`: per-stage events.
+static int32_t run_keys_sort(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order, uint32_t key_bits,
+                             const BatchPlan &pl, const float *rays_dev, uint64_t n, void *keys, void *ws, uint32_t *perm,
+                             cudaStream_t s, bool events, uint32_t **slot) {
     int32_t rc = HCC_OK;
+    *slot = nullptr;
     if (events) HCC_CUDA_TRY(cudaEventRecord(p->ev[1], s));
-    if (order == HCC_ORDER_HCC) rc = encode_launch(rays_dev, n, cut, p->d_keys, s, first);
-    else if (order == HCC_ORDER_TWOPOINT) rc = encode_twopoint_launch(rays_dev, n, bvh->scene_lo, bvh->scene_hi, key_bits, p->d_keys, s, first);
+    if (order == HCC_ORDER_HCC) rc = encode_launch(rays_dev, n, cut, keys, s, LK_FIRST);
+    else if (order == HCC_ORDER_TWOPOINT) rc = encode_twopoint_launch(rays_dev, n, bvh->scene_lo, bvh->scene_hi, key_bits, keys, s, LK_FIRST);
     if (rc != HCC_OK) return rc;
     if (events) HCC_CUDA_TRY(cudaEventRecord(p->ev[2], s));
-    uint32_t *slot = nullptr;
-    if (order != HCC_ORDER_NOSORT && n != 0) {
-        const uint32_t lo = p->sort_skip_bits < bits_used ? p->sort_skip_bits : bits_used;
-        slot = trace_take_slot(bvh);
-        rc = sort_launch(p->d_keys, n, container, lo, bits_used, perm, p->d_ws, p->ws_bytes, s, slot, LK_CHAIN);
+    if (n != 0) {
+        *slot = trace_take_slot(bvh);
+        if (order != HCC_ORDER_NOSORT) {
+            const uint32_t lo = p->sort_skip_bits < pl.bits_used ? p->sort_skip_bits : pl.bits_used;
+            rc = sort_launch(keys, n, pl.container, lo, pl.bits_used, perm, ws, p->ws_bytes, s, *slot, LK_CHAIN);
+        } else {
+            rc = trace_arm(*slot, s);
+        }
         if (rc != HCC_OK) return rc;
     }
     if (events) HCC_CUDA_TRY(cudaEventRecord(p->ev[3], s));
-    rc = trace_launch("hcc_reorder_trace", bvh, rays_dev, n, order == HCC_ORDER_NOSORT ? nullptr : perm, mode, hits_dev, nullptr, s,
-                      slot, first);
-    if (rc != HCC_OK) return rc;
-    if (events) HCC_CUDA_TRY(cudaEventRecord(p->ev[4], s));
     return HCC_OK;
 }
 
@@ -153,9 +171,17 @@ extern "C" int32_t hcc_reorder_trace(hcc_pipeline *p, const hcc_bvh *bvh, const 
     HCC_REQUIRE(p && bvh, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: NULL handle");
     cudaStream_t s = (cudaStream_t)stream;
     p->timed = false;
-    int32_t rc = run_chain(p, bvh, cut, order, key_bits, rays_dev, n, mode, hits_dev, perm_out_dev ? perm_out_dev : p->d_perm[0], s,
-                           LK_FIRST, p->timing);
+    BatchPlan pl;
+    int32_t rc = plan_batch(p, cut, order, key_bits, n, mode, &pl);
     if (rc != HCC_OK) return rc;
+    uint32_t *perm = perm_out_dev ? perm_out_dev : p->d_perm[0], *slot = nullptr;
+    rc = run_keys_sort(p, bvh, cut, order, key_bits, pl, rays_dev, n, p->d_keys, p->d_ws, perm, s, p->timing, &slot);
+    if (rc != HCC_OK) return rc;
+    // the trace kernel: a chained launch behind the kernel that zeroed its counter
+    rc = trace_launch("hcc_reorder_trace", bvh, rays_dev, n, order == HCC_ORDER_NOSORT ? nullptr : perm, mode, hits_dev, nullptr, s,
+                      slot, LK_CHAIN);
+    if (rc != HCC_OK) return rc;
+    if (p->timing) HCC_CUDA_TRY(cudaEventRecord(p->ev[4], s));
     p->timed = p->timing;
     p->timed_host = false;
     p->last_stream = s;
@@ -163,23 +189,56 @@ extern "C" int32_t hcc_reorder_trace(hcc_pipeline *p, const hcc_bvh *bvh, const 
     return HCC_OK;
 }
 
-// Both batches of one bounce in one call (PAPER.md:245-247 runs the three kernels per batch; a renderer has the
-// diffuse and the shadow batch of a bounce at the same time).  The second batch's chain starts with a dependent launch
-// that does NOT wait: it is encoded and sorted while the first batch's traversal kernel runs out (its last rays leave
-// most SMs idle), and its own traversal starts as soon as its permutation is complete.  Safe by construction: the second
-// chain's first kernel is launched only after the first batch's trace kernel has passed its own wait, so everything
-// before that trace is complete; the trace reads none of the buffers the second chain writes (keys, sort workspace, the
-// second permutation buffer, its own work counter, its own hits).  The first kernel of the NEXT call on this stream is a
-// plain launch and therefore ordered after both traces.  Both batches must be complete in memory when the call is made.
+static int32_t ensure_side(hcc_pipeline *p) {
+    if (p->side) return HCC_OK;
+    cudaError_t e = cudaMalloc(&p->d_keys2, (size_t)(p->container_bits_max / 8) * p->n_max);
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_ws2, p->ws_bytes);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking);
+    if (e != cudaSuccess) {
+        set_error("hcc_reorder_trace_pair: %s", cudaGetErrorString(e));
+        return e == cudaErrorMemoryAllocation ? HCC_ERR_OUT_OF_MEMORY : HCC_ERR_CUDA;
+    }
+    return HCC_OK;
+}
+
+// Both batches of one bounce in one call (PAPER.md:245-247 runs the three kernels per batch; a renderer has the diffuse
+// and the shadow batch of a bounce at the same time).  Schedule:
+//   stream s    : keys + sort of batch a  --+--> trace a --> trace b (dependent launch that does NOT wait for trace a)
+//   side stream : keys + sort of batch b  --+   (forked from s and joined back into it by events)
+// The two sorts are chains of small latency-bound kernels that fill each other's gaps; the traversal kernel of batch b
+// becomes resident CTA by CTA as that of batch a runs out (its last rays leave most SMs idle), because its inputs - the
+// permutation and the zeroed work counter - were complete before trace a was launched.  The two batches use scratch of
+// their own (keys, sort workspace, permutation, counter, hits).  The first kernel of the NEXT call on s is a plain launch,
+// ordered after both traces; the side stream is touched again only behind an event recorded on s after them.
 extern "C" int32_t hcc_reorder_trace_pair(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order, uint32_t key_bits,
                                           const float *rays_a_dev, uint64_t n_a, int32_t mode_a, void *hits_a_dev,
                                           const float *rays_b_dev, uint64_t n_b, int32_t mode_b, void *hits_b_dev, void *stream) {
     HCC_REQUIRE(p && bvh, HCC_ERR_INVALID_ARG, "hcc_reorder_trace_pair: NULL handle");
     cudaStream_t s = (cudaStream_t)stream;
     p->timed = false;
-    int32_t rc = run_chain(p, bvh, cut, order, key_bits, rays_a_dev, n_a, mode_a, hits_a_dev, p->d_perm[0], s, LK_FIRST, false);
+    BatchPlan pa, pb;
+    int32_t rc = plan_batch(p, cut, order, key_bits, n_a, mode_a, &pa);
+    if (rc == HCC_OK) rc = plan_batch(p, cut, order, key_bits, n_b, mode_b, &pb);
+    if (rc == HCC_OK) rc = ensure_side(p);
     if (rc != HCC_OK) return rc;
-    rc = run_chain(p, bvh, cut, order, key_bits, rays_b_dev, n_b, mode_b, hits_b_dev, p->d_perm[1], s, n_a ? LK_OVERLAP : LK_FIRST, false);
+    uint32_t *slot_a = nullptr, *slot_b = nullptr;
+    HCC_CUDA_TRY(cudaEventRecord(p->ev_fork, s));
+    HCC_CUDA_TRY(cudaStreamWaitEvent(p->side, p->ev_fork, 0));
+    rc = run_keys_sort(p, bvh, cut, order, key_bits, pb, rays_b_dev, n_b, p->d_keys2, p->d_ws2, p->d_perm[1], p->side, false, &slot_b);
+    if (rc == HCC_OK) rc = run_keys_sort(p, bvh, cut, order, key_bits, pa, rays_a_dev, n_a, p->d_keys, p->d_ws, p->d_perm[0], s, false, &slot_a);
+    // join even after an error, so the side stream never runs ahead of the caller's stream unnoticed
+    cudaError_t e = cudaEventRecord(p->ev_join, p->side);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s, p->ev_join, 0);
+    if (rc != HCC_OK) return rc;
+    HCC_CUDA_TRY(e);
+    const bool sorted = order != HCC_ORDER_NOSORT;
+    rc = trace_launch("hcc_reorder_trace_pair", bvh, rays_a_dev, n_a, sorted ? p->d_perm[0] : nullptr, mode_a, hits_a_dev, nullptr, s,
+                      slot_a, LK_FIRST);
+    if (rc != HCC_OK) return rc;
+    rc = trace_launch("hcc_reorder_trace_pair", bvh, rays_b_dev, n_b, sorted ? p->d_perm[1] : nullptr, mode_b, hits_b_dev, nullptr, s,
+                      slot_b, n_a ? LK_OVERLAP : LK_FIRST);
     if (rc != HCC_OK) return rc;
     p->timed_host = false;
     p->last_stream = s;

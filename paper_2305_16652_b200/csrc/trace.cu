@@ -170,6 +170,7 @@ struct TraceScene {
     const uint32_t *wrec;
     const float4 *ttri;
     uint32_t root_ref;
+    uint32_t wait;      // call griddepcontrol.wait before the first global access (0: a dependent launch that overlaps its predecessor)
     float q_lo[3], q_scale[3];
 };
 
@@ -215,7 +216,7 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
 
     if (lane == 0) sts32(sa_tail, 0u);
     __syncwarp();
-    pdl_wait();          // the permutation (or whatever wrote the rays) and the zeroed work counter are complete
+    if (sc.wait) pdl_wait();   // the permutation (or whatever wrote the rays) and the zeroed work counter are complete
     pdl_trigger();
 #ifdef HCC_TRACE_TIMELINE   // debug builds only: per-warp start / exhaustion / end times behind the eight counters
     unsigned long long tl_t0 = 0, tl_ex = 0;
@@ -517,6 +518,11 @@ uint32_t *hcc::trace_take_slot(const hcc_bvh *bvh) {
     return bvh->d_trace_ctl + 2u * (bvh->trace_calls->fetch_add(1u) % (uint32_t)HCC_TRACE_SLOTS);
 }
 
+int32_t hcc::trace_arm(uint32_t *slot, cudaStream_t s) {
+    HCC_CUDA_TRY(launch_k(LK_FIRST, k_trace_arm, dim3(1), dim3(32), 0, s, slot, 1));
+    return HCC_OK;
+}
+
 int32_t hcc::trace_launch(const char *who, const hcc_bvh *bvh, const float *rays_dev, uint64_t n, const uint32_t *perm_dev,
                           int32_t mode, void *hits_dev, unsigned long long *stats_dev, cudaStream_t s, uint32_t *armed_slot,
                           LaunchKind kind) {
@@ -534,11 +540,16 @@ int32_t hcc::trace_launch(const char *who, const hcc_bvh *bvh, const float *rays
     TraceScene sc;
     sc.wrec = bvh->d_wrec; sc.ttri = bvh->d_ttri; sc.root_ref = bvh->root_ref;
     for (int a = 0; a < 3; ++a) { sc.q_lo[a] = bvh->q_lo[a]; sc.q_scale[a] = bvh->q_scale[a]; }
+    // an armed slot: the trace kernel itself is launched as `kind`; else a one-warp kernel launched as `kind` arms a
+    // fresh slot and the trace kernel is a chained launch behind it
     uint32_t *ctl = armed_slot;
+    LaunchKind trace_kind = kind;
     if (!ctl) {
         ctl = trace_take_slot(bvh);
         HCC_CUDA_TRY(launch_k(kind, k_trace_arm, dim3(1), dim3(32), 0, s, ctl, kind_waits(kind)));
+        trace_kind = LK_CHAIN;
     }
+    sc.wait = (uint32_t)kind_waits(trace_kind);
     const float4 *rays = (const float4 *)rays_dev;
     const bool any = mode == HCC_TRACE_ANY;
 #ifdef HCC_TRACE_TIMELINE   // debug builds: the plain kernel writes its per-warp times behind the counters
@@ -546,7 +557,7 @@ int32_t hcc::trace_launch(const char *who, const hcc_bvh *bvh, const float *rays
 #else
     auto kern = stats_dev ? (any ? k_trace<true, true> : k_trace<false, true>) : (any ? k_trace<true, false> : k_trace<false, false>);
 #endif
-    HCC_CUDA_TRY(launch_k(LK_CHAIN, kern, dim3(blocks), dim3(TRACE_THREADS), 0, s, sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, stats_dev));
+    HCC_CUDA_TRY(launch_k(trace_kind, kern, dim3(blocks), dim3(TRACE_THREADS), 0, s, sc, rays, perm_dev, (uint32_t)n, hits_dev, ctl, stats_dev));
     return HCC_OK;
 }
 
