@@ -321,7 +321,7 @@ def run_ours(args):
             shadow = shadow[torch.randperm(sc.n_s, device="cuda", generator=g)].contiguous()
         sc.batches = ((diffuse, hcc.TRACE_CLOSEST, "diffuse"), (shadow, hcc.TRACE_ANY, "shadow"))
         if getattr(sc, "pipe", None) is None or sc.pipe.n_max < max(sc.n_d, sc.n_s):
-            sc.pipe = hcc.Pipeline(max(sc.n_d, sc.n_s), 64, host_staging=(sc.name == args.workload))
+            sc.pipe = hcc.Pipeline(max(sc.n_d, sc.n_s), 64)
         sc.hits = {"diffuse": torch.empty((sc.n_d, 4), dtype=torch.float32, device="cuda"),
                    "shadow": torch.empty(sc.n_s, dtype=torch.uint8, device="cuda")}
 
@@ -716,21 +716,30 @@ def run_ours(args):
     hits_pin = {"diffuse": torch.empty((n_d, 4), dtype=torch.float32).pin_memory(),
                 "shadow": torch.empty(n_s, dtype=torch.uint8).pin_memory()}
 
-    # one pipeline and one stream per batch: the shadow batch's host->device copy overlaps the diffuse
-    # batch's kernels, the diffuse hits go back while the shadow batch is traced
-    pipes_h = {"diffuse": hcc.Pipeline(n_d, 64, host_staging=True), "shadow": pipe}
-    streams_h = {"diffuse": torch.cuda.Stream(), "shadow": torch.cuda.Stream()}
+    # the batches are streamed in chunks of about half a million rays, each through a pipeline and a stream of its own
+    # (hcc_reorder_trace_host_async: copy in, encode, sort, trace, copy out): the host->device copies queue up on the copy
+    # engine back to back while the kernels of the chunks already on the device run, and hits go back as chunks finish.
+    # A chunk is sorted within itself (coherence is made per chunk); hits do not depend on the order.
+    e2e_chunk = max(1, args.e2e_chunk)
+    chunks = []           # (name, mode, start, stop)
+    for _, mode, name in sc.batches:
+        nb = nrays[name]
+        parts = max(1, (nb + e2e_chunk - 1) // e2e_chunk)
+        for k in range(parts):
+            a_, b_ = shard.ray_shard(nb, k, parts)
+            chunks.append((name, mode, a_, b_))
+    pipes_h = [hcc.Pipeline(max(b_ - a_, 1), 64, host_staging=True) for _, _, a_, b_ in chunks]
+    streams_h = [torch.cuda.Stream() for _ in chunks]
 
     def step_host():
         cur = torch.cuda.current_stream()
-        for _, mode, name in sc.batches:
-            st = streams_h[name]
+        for (name, mode, a_, b_), ph, st in zip(chunks, pipes_h, streams_h):
             st.wait_stream(cur)
-            pipes_h[name].reorder_trace_host_async(bvh, cut, hcc.ORDER_HCC, rays_pin[name], hits_pin[name], mode,
-                                                   key_bits=w.key_bits, stream=st)
-        for name in ("diffuse", "shadow"):
-            pipes_h[name].synchronize()
-            cur.wait_stream(streams_h[name])
+            ph.reorder_trace_host_async(bvh, cut, hcc.ORDER_HCC, rays_pin[name][a_:b_], hits_pin[name][a_:b_], mode,
+                                        key_bits=w.key_bits, stream=st)
+        for ph, st in zip(pipes_h, streams_h):
+            ph.synchronize()
+            cur.wait_stream(st)
     for _ in range(3):
         step_host()
     torch.cuda.synchronize()
@@ -750,7 +759,8 @@ def run_ours(args):
     step(sc, hcc.ORDER_HCC)
     assert torch.equal(hits_pin["shadow"].cuda(), hits_s) and torch.equal(hits_pin["diffuse"].cuda().view(torch.int32), hits_d.view(torch.int32))
     e2e = {"value": world * n / e2e_ms / 1e3, "unit": UNIT, "ms_per_step": e2e_ms,
-           "h2d_bytes_per_step": 32 * n, "d2h_bytes_per_step": 16 * n_d + n_s}
+           "h2d_bytes_per_step": 32 * n, "d2h_bytes_per_step": 16 * n_d + n_s,
+           "how": f"{len(chunks)} chunks of <= {e2e_chunk} rays, one hcc_reorder_trace_host_async each on a stream of its own"}
 
     # kernels launched per step: per batch 1 key kernel + (init + histogram + scan + one per digit) + 1 trace
     launches_per_step = 2 * (1 + (3 + passes) + 1)
@@ -808,6 +818,7 @@ def main():
     ap.add_argument("--no-large-n", action="store_true", help="skip the large-batch encode/sort roofline leg")
     ap.add_argument("--configs", default="fig1,large", help="comma list of further configs to run at their stated sizes (fig1,large): other_configs")
     ap.add_argument("--counters-all", action="store_true", help="per-order trace counters for --configs too")
+    ap.add_argument("--e2e-chunk", type=int, default=1 << 19, help="rays per chunk of the host-buffer (e2e) leg")
     ap.add_argument("--quick", action="store_true", help="skip the later-bounce and shuffled-input legs")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":

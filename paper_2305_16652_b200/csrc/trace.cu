@@ -25,12 +25,15 @@
 
 namespace hcc {
 
-constexpr int TRACE_THREADS = 128;
-#ifndef HCC_TRACE_BLOCKS_PER_SM       // closest hit: CTAs of 128 threads per SM
-#define HCC_TRACE_BLOCKS_PER_SM 7
+#ifndef HCC_TRACE_THREADS             // threads of a CTA: 32, 64 or 128 (the warps of a CTA share nothing but its lifetime)
+#define HCC_TRACE_THREADS 128
+#endif
+constexpr int TRACE_THREADS = HCC_TRACE_THREADS;
+#ifndef HCC_TRACE_BLOCKS_PER_SM       // closest hit: CTAs per SM
+#define HCC_TRACE_BLOCKS_PER_SM (7 * 128 / HCC_TRACE_THREADS)
 #endif
 #ifndef HCC_TRACE_BLOCKS_PER_SM_ANY
-#define HCC_TRACE_BLOCKS_PER_SM_ANY 7
+#define HCC_TRACE_BLOCKS_PER_SM_ANY (7 * 128 / HCC_TRACE_THREADS)
 #endif
 #ifndef HCC_TRACE_REFILL_AT
 #define HCC_TRACE_REFILL_AT 8
@@ -65,11 +68,13 @@ constexpr uint32_t QCAP = 256;
 //                lowered by committed hits), closest: key ord(t) << 32 | prim at +32 and (u, v) at +40;
 //                any: occluded flag at +32
 //   leaf queues: QCAP x 8 bytes per warp: (leaf reference, owner lane); queue tails: one word per warp
-//   stacks     : SMEM_STACK rows of 128 words (a lane's entries are 512 bytes apart: conflict-free)
+//   stacks     : SMEM_STACK rows of one word per thread (a lane's entries are ROW bytes apart: conflict-free)
 constexpr uint32_t SLOT_BYTES = 48;
+constexpr uint32_t ROW = 4u * TRACE_THREADS, ROW_SHIFT = TRACE_THREADS == 128 ? 9u : TRACE_THREADS == 64 ? 8u : 7u;
+static_assert(TRACE_THREADS == 32 || TRACE_THREADS == 64 || TRACE_THREADS == 128, "CTA size");
 constexpr uint32_t OFF_SLOTS = 0, OFF_QUEUE = OFF_SLOTS + SLOT_BYTES * TRACE_THREADS,
                    OFF_TAIL = OFF_QUEUE + 8 * QCAP * TRACE_WARPS, OFF_STACK = OFF_TAIL + 16,
-                   SMEM_BYTES = OFF_STACK + 512 * SMEM_STACK;
+                   SMEM_BYTES = OFF_STACK + ROW * SMEM_STACK;
 static_assert(TRACE_WARPS <= 4, "queue tails: one word per warp in 16 bytes");
 
 __device__ __forceinline__ uint32_t lds32(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
@@ -197,7 +202,7 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
     const uint32_t sa_wslots = sa + OFF_SLOTS + SLOT_BYTES * (tid & ~31u);       // slot of lane 0 of the warp
     const uint32_t sa_queue = sa + OFF_QUEUE + 8u * QCAP * (tid >> 5);
     const uint32_t sa_tail = sa + OFF_TAIL + 4u * (tid >> 5);
-    const uint32_t st_base = sa + OFF_STACK + 4u * tid, st_limit = st_base + 512u * SMEM_STACK;
+    const uint32_t st_base = sa + OFF_STACK + 4u * tid, st_limit = st_base + ROW * SMEM_STACK;
     unsigned long long n_nodes = 0, n_tris = 0, n_rays = 0, n_sect = 0, n_steps = 0, n_lanes = 0, n_rounds = 0;
     uint32_t max_sp = 0;
 
@@ -224,13 +229,13 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
 #endif
 
     auto push = [&](uint32_t v) {      // general form (the node step has its own fast path)
-        if (sp < st_limit) sts32(sp, v); else l_stack[(sp - st_limit) >> 9] = v;
-        sp += 512u;
+        if (sp < st_limit) sts32(sp, v); else l_stack[(sp - st_limit) >> ROW_SHIFT] = v;
+        sp += ROW;
     };
     auto pop = [&]() -> uint32_t {
         if (sp == st_base) return 0u;
-        sp -= 512u;
-        return sp < st_limit ? lds32(sp) : l_stack[(sp - st_limit) >> 9];
+        sp -= ROW;
+        return sp < st_limit ? lds32(sp) : l_stack[(sp - st_limit) >> ROW_SHIFT];
     };
 
     // one triangle round: the ROUND_LEAVES leaves at the head of the queue, LPL lanes per leaf; lane k of a
@@ -381,7 +386,7 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
                 const uint32_t peers = __match_any_sync(0xFFFFFFFFu, cur != 0u ? cur : (0x40000000u | lane));
                 if (cur != 0u && (peers & lanes_below) == 0u) ++n_sect;
                 if (lane == 0) { ++n_steps; n_lanes += __popc(wm); }
-                max_sp = max(max_sp, (sp - st_base) >> 9);
+                max_sp = max(max_sp, (sp - st_base) >> ROW_SHIFT);
             }
             if (cur != 0u) {
                 const uint32_t *rec = sc.wrec + 16 * (size_t)(cur - 1u);
@@ -446,14 +451,14 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
                     hP1 = (i0 || i1) && i2; rP1 = r2;
                     hP0 = (i0 || i1 || i2) && i3; rP0 = r3;
                 }
-                if (sp + 3u * 512u <= st_limit) {
+                if (sp + 3u * ROW <= st_limit) {
                     // all in shared memory: store unconditionally, advance if the child was hit
-                    sts32(sp, rP0); sp += hP0 ? 512u : 0u;
-                    sts32(sp, rP1); sp += hP1 ? 512u : 0u;
-                    sts32(sp, rP2); sp += hP2 ? 512u : 0u;
+                    sts32(sp, rP0); sp += hP0 ? ROW : 0u;
+                    sts32(sp, rP1); sp += hP1 ? ROW : 0u;
+                    sts32(sp, rP2); sp += hP2 ? ROW : 0u;
                     if (hW) cur = rW;
                     else if (sp == st_base) cur = 0u;
-                    else { sp -= 512u; cur = lds32(sp); }
+                    else { sp -= ROW; cur = lds32(sp); }
                 } else {
                     if (hP0) push(rP0);
                     if (hP1) push(rP1);
