@@ -315,7 +315,7 @@ HCC_API int32_t hcc_reorder_trace_host_async(hcc_pipeline *p, const hcc_bvh *bvh
                                      void *hits_host, void *stream);
 /* Both batches of one bounce in one call: batch a (say the diffuse rays, HCC_TRACE_CLOSEST) and batch b (the
  * shadow rays, HCC_TRACE_ANY) go through the same three kernels as in hcc_reorder_trace, scheduled so that they
- * fill each other's gaps: b's keys and sort run on a stream of the pipeline's own beside a's (forked from and
+ * fill each other's gaps: up to 2^23 rays in total, b's keys and sort run on a stream of the pipeline's own beside a's (forked from and
  * joined back into `stream` by events), then a's traversal kernel and, as a dependent launch that does not wait
  * for it, b's: b's CTAs become resident as a's run out.  Both batches must be complete in memory when the call
  * is made.  Results are those of two hcc_reorder_trace calls.  Either n may be 0.  The first call allocates a

@@ -1,5 +1,6 @@
 """Parity at BASELINE.json's full sizes, through the call bench.py times (hcc_reorder_trace on whole
-batches): config 2 in full (1,048,576 + 2,097,152 rays) and config 3 in full (16.6 M + 33.2 M rays).
+batches, then both at once through hcc_reorder_trace_pair): config 2 in full (1,048,576 + 2,097,152 rays), config 3 in
+full (16.6 M + 33.2 M rays) and config 5 in full (33.2 M + 66.4 M rays).
 The oracle cannot run these batches whole, so: keys and hits of a seeded SAMPLE of rays are compared
 with the oracle one by one (bit-exact keys, hits within the north_star's bars), and the permutation
 is checked by the properties that define it at any size (a permutation; keys non-decreasing along
@@ -38,6 +39,7 @@ def _run(hcc, name, bounce, res_scale=1.0):
     assert np.array_equal(ent, tables.entry_node) and np.array_equal(cnt, tables.table_cnt)
     info = cut.info()
     pipe = hcc.Pipeline(shadow.shape[0], 64)
+    kept = []
     for rays_h, mode in ((diffuse, hcc.TRACE_CLOSEST), (shadow, hcc.TRACE_ANY)):
         n = rays_h.shape[0]
         rays = torch.from_numpy(rays_h).cuda()
@@ -73,7 +75,14 @@ def _run(hcc, name, bounce, res_scale=1.0):
         else:
             occ = hits[torch.from_numpy(idx).cuda()].cpu().numpy()
             assert np.array_equal(occ, oracle.any_bvh(sub, b.nodes, b.prim_idx, b.tris))
-        del rays, perm, hits, keys
+        kept.append((rays, mode, hits))
+        del perm, keys
+    # the call bench.py times: both batches in ONE hcc_reorder_trace_pair (the second traversal kernel overlapping the
+    # first one's tail, the key and sort kernels side by side on two streams) gives the same hits bit for bit
+    (ra, ma, ha), (rb, mb, hb) = kept
+    pa, pb = torch.empty_like(ha), torch.empty_like(hb)
+    pipe.reorder_trace_pair(bvh, cut, hcc.ORDER_HCC, ra, ma, pa, rb, mb, pb, key_bits=w.key_bits)
+    assert torch.equal(pa.view(torch.uint8), ha.view(torch.uint8)) and torch.equal(pb, hb)
     return diffuse.shape[0], shadow.shape[0]
 
 
@@ -96,9 +105,9 @@ def test_config3_full_size_second_bounce(hcc):
     assert n_d > 16_000_000 and n_s > 32_000_000
 
 
-def test_config5_scene_in_full_at_quarter_resolution(hcc):
-    """Config 5's scene in full (10.8 M triangles, 7.1 M nodes: a BVH far larger than L2, traversal
-    stacks deeper than the 16 shared-memory entries) with 480x270x16 primaries: K = 16,384, 64-bit
+def test_config5_full_size(hcc):
+    """Config 5 at its stated size: 10.8 M triangles, 7.1 M nodes (a BVH far larger than L2, traversal stacks deeper
+    than the shared-memory rows), 1920x1080x16 primaries -> 33.2 M diffuse + 66.4 M shadow rays: K = 16,384, 64-bit
     keys 16x16x8x8."""
-    n_d, n_s = _run(hcc, "large", 1, res_scale=0.25)
-    assert n_d > 2_000_000 and n_s == 2 * n_d
+    n_d, n_s = _run(hcc, "large", 1)
+    assert n_d > 33_000_000 and n_s == 2 * n_d
