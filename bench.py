@@ -814,7 +814,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--bounce", type=int, default=1, help="which bounce's ray batches to run (1 = rays off the primary hits)")
     ap.add_argument("--res-scale", type=float, default=1.0, help="image scale of the workload (1.0 = the config's resolution)")
-    ap.add_argument("--studies", action="store_true", help="add the NEXT-row studies: sort truncation, lambda/ANC, grid and PPC orders")
+    ap.add_argument("--studies", action="store_true", default=True,
+                    help="the NEXT-row studies: sort truncation, lambda/ANC, grid and PPC orders, config-4 sweep (on by default)")
+    ap.add_argument("--no-studies", dest="studies", action="store_false", help="skip the studies (about 45 s)")
     ap.add_argument("--no-large-n", action="store_true", help="skip the large-batch encode/sort roofline leg")
     ap.add_argument("--configs", default="fig1,large", help="comma list of further configs to run at their stated sizes (fig1,large): other_configs")
     ap.add_argument("--counters-all", action="store_true", help="per-order trace counters for --configs too")
