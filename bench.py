@@ -260,9 +260,17 @@ def run_ours(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    # HCC_BENCH_SHARED_GPU=1 (code-path check on a one-GPU box, never a measurement): the ranks share the GPUs there are and
+    # talk over gloo; no rank's kernels wait on another's, the collectives are the barrier, two reductions and one gather
+    shared_gpu = os.environ.get("HCC_BENCH_SHARED_GPU") == "1"
+    if shared_gpu:
+        local %= torch.cuda.device_count()
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if shared_gpu:
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     hbm_gbs, sm_max_mhz, peak_kind = _peaks()
     alu_peak = SM_COUNT * LANES_PER_SM * sm_max_mhz * 1e6 / 1e12     # T lane-op/s
     ev = lambda: torch.cuda.Event(enable_timing=True)
@@ -271,7 +279,7 @@ def run_ours(args):
     def max_over_ranks(x):
         if world == 1:
             return float(x)
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        t = torch.tensor([x], dtype=torch.float64, device="cpu" if shared_gpu else "cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
 
@@ -795,7 +803,8 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
-            "config": _config(args, w, n_d, n_s, l2="flushed between timed steps (256 MiB write)", world=world),
+            "config": dict(_config(args, w, n_d, n_s, l2="flushed between timed steps (256 MiB write)", world=world),
+                           **({"shared_gpu_code_path_check": True} if shared_gpu else {})),
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
             "roofline": roof, "cpu_baseline": cpu,
             "cut": {"widths": info["widths"], "K_eff": info["K_eff"], "bits_used": info["bits_used"],

@@ -109,3 +109,27 @@ def test_sharded_product_path_on_one_gpu(world, tiny):
             assert torch.equal(gather_hits(parts[0], n).view(torch.uint8), whole.view(torch.uint8))
         finally:
             dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+def test_bench_two_ranks_code_path_on_one_gpu():
+    """`python bench.py --gpus 2` starts its own two ranks (torch.distributed.run); with HCC_BENCH_SHARED_GPU=1 they share the
+    test box's one GPU and talk over gloo (a code-path check, not a measurement: no rank's kernels wait on another's).  The line
+    must come from two ranks, and the strong-scaling leg's gathered hits (product kernels on each rank's shard.ray_shard range)
+    must equal the unsharded trace."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, HCC_BENCH_SHARED_GPU="1")
+    for k in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT"):
+        env.pop(k, None)
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--workload", "tiny", "--steps", "3", "--configs=",
+                        "--no-studies", "--no-cpu-baseline", "--no-large-n", "--quick"], capture_output=True, text=True, env=env,
+                       timeout=600, cwd=root)
+    assert r.returncode == 0, r.stderr[-2000:]
+    line = json.loads([l for l in r.stdout.splitlines() if l.startswith("{")][-1])
+    assert line["n_gpus"] == 2 and line["config"]["shared_gpu_code_path_check"] is True
+    s = line["strong_scaling"]
+    assert s["ranks"] == 2 and s["scaling"] == "strong" and s["gathered_hits_equal_unsharded"] is True
+    assert s["rays_total"] == line["config"]["diffuse_rays"] + line["config"]["shadow_rays"]
