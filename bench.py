@@ -44,6 +44,10 @@ UNIT = "Mrays/s"
 #          conversions, 24 fma, 16 min/max, 4 compares, trace.cu) + 36 per triangle test (the formula in
 #          include/hcc.h); encode: 26 per exact fp32 slab test (6 sub, 6 mul, 12 min/max, compare, bit).
 OPS_BOX, OPS_NODE, OPS_TRI = 26, 68, 36
+# the same operations weighted by the issue cycles their pipe takes (B300_MICROARCH.md: min/max, compare, select, PRMT run on the
+# ALU pipe at 16 lanes per scheduler and clock = 2 cycles per warp instruction; fma/mul/add at 1): per wide record 44 ALU-pipe
+# operations + 24 fma = 112 issue cycles' worth; per triangle test 10 compares/selects + 26 fma/mul/add = 46
+CYC_NODE, CYC_TRI = 2 * 44 + 24, 2 * 10 + 26
 SM_COUNT, LANES_PER_SM = 148, 128
 TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_trace_traffic.md")
 KERNEL_SOURCES = ("paper_2305_16652_b200/csrc/trace.cu", "paper_2305_16652_b200/csrc/bvh.cu",
@@ -419,7 +423,8 @@ def run_ours(args):
                 o[on] = {"node_records_per_ray": st["nodes"] / max(st["rays"], 1), "tri_tests_per_ray": st["tris"] / max(st["rays"], 1),
                          "distinct_records_per_warp_step": st["records_per_step"], "lanes_per_warp_step": st["lanes_per_step"],
                          "tri_tests_per_round": st["tri_tests_per_round"], "max_stack": st["max_stack"],
-                         "lane_ops": st["nodes"] * OPS_NODE + st["tris"] * OPS_TRI}
+                         "lane_ops": st["nodes"] * OPS_NODE + st["tris"] * OPS_TRI,
+                         "lane_cycles": st["nodes"] * CYC_NODE + st["tris"] * CYC_TRI}
             out[name] = {"anc_hcc": hcc.anc(keys0, perms["hcc"]), "anc_nosort": hcc.anc(keys0, None), "orders": o}
         return out
 
@@ -537,7 +542,8 @@ def run_ours(args):
             "sort": {"bound": "hbm", "achieved": sort_gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": sort_gbs / hbm_gbs,
                      "passes": passes, "bytes_per_pair_moved": sb_real, "bytes_per_pair_survey": sb_algo,
                      "frac_survey_bytes": nb * sb_algo / (o["sort_ms"] * 1e-3) / 1e9 / hbm_gbs},
-            "trace": {"bound": "alu", "achieved": tr, "peak": alu_peak, "unit": "Tlaneop/s", "frac": tr / alu_peak}}
+            "trace": {"bound": "alu", "achieved": tr, "peak": alu_peak, "unit": "Tlaneop/s", "frac": tr / alu_peak,
+                      "frac_pipe_weighted": diag[name]["orders"]["hcc"]["lane_cycles"] / (o["trace_ms"] * 1e-3) / 1e12 / alu_peak}}
     # dominant kernel of the step
     dom = max((("diffuse", "trace"), ("shadow", "trace"), ("diffuse", "sort"), ("shadow", "sort"),
                ("diffuse", "encode"), ("shadow", "encode")), key=lambda k: orders["hcc"][k[0]][k[1] + "_ms"])
