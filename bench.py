@@ -333,7 +333,7 @@ def run_ours(args):
             shadow = shadow[torch.randperm(sc.n_s, device="cuda", generator=g)].contiguous()
         sc.batches = ((diffuse, hcc.TRACE_CLOSEST, "diffuse"), (shadow, hcc.TRACE_ANY, "shadow"))
         if getattr(sc, "pipe", None) is None or sc.pipe.n_max < max(sc.n_d, sc.n_s):
-            sc.pipe = hcc.Pipeline(max(sc.n_d, sc.n_s), 64)
+            sc.pipe = hcc.Pipeline(max(sc.n_d, sc.n_s), 64, pair=True)
         sc.hits = {"diffuse": torch.empty((sc.n_d, 4), dtype=torch.float32, device="cuda"),
                    "shadow": torch.empty(sc.n_s, dtype=torch.uint8, device="cuda")}
 

@@ -281,9 +281,13 @@ HCC_API int32_t hcc_trace_stats(const hcc_bvh *bvh, const float *rays_dev, uint6
 /* ---- the per-batch path as one call -----------------------------------------------------
  * PAPER.md:245-247 (Figure 11): key compute kernel -> ray sort kernel -> trace kernel, per
  * ray batch.  A pipeline handle owns the scratch for batches of up to n_max rays (keys, perm,
- * the sort workspace, and with host_staging != 0 a device copy of the rays and hits), so a
- * call allocates nothing.  container_bits_max: 32 or 64 = widest key it must hold. */
-HCC_API int32_t hcc_pipeline_create(uint64_t n_max, uint32_t container_bits_max, uint32_t host_staging,
+ * the sort workspace; with HCC_PIPELINE_HOST_STAGING a device copy of the rays and hits for the
+ * host-buffer calls; with HCC_PIPELINE_PAIR a second key buffer and sort workspace, a stream
+ * and two events for hcc_reorder_trace_pair), so a call allocates nothing.
+ * container_bits_max: 32 or 64 = widest key it must hold.  flags: OR of HCC_PIPELINE_*. */
+#define HCC_PIPELINE_HOST_STAGING 1u
+#define HCC_PIPELINE_PAIR 2u
+HCC_API int32_t hcc_pipeline_create(uint64_t n_max, uint32_t container_bits_max, uint32_t flags,
                             hcc_pipeline **out);
 HCC_API int32_t hcc_pipeline_destroy(hcc_pipeline *p);
 /* Low key bits the pipeline's sort leaves unordered (hcc_sort_range's bit_lo);
@@ -302,7 +306,7 @@ HCC_API int32_t hcc_reorder_trace(hcc_pipeline *p, const hcc_bvh *bvh, const hcc
                           void *hits_dev, uint32_t *perm_out_dev, void *stream);
 /* The same with HOST buffers: copies rays_host (32 n bytes; pinned memory makes the copy
  * asynchronous) to the device, runs the batch, copies the hits (16 n bytes CLOSEST, n bytes
- * ANY) to hits_host and synchronises `stream` before returning.  Needs host_staging. */
+ * ANY) to hits_host and synchronises `stream` before returning.  Needs HCC_PIPELINE_HOST_STAGING. */
 HCC_API int32_t hcc_reorder_trace_host(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
                                uint32_t key_bits, const float *rays_host, uint64_t n, int32_t mode,
                                void *hits_host, void *stream);
@@ -318,8 +322,8 @@ HCC_API int32_t hcc_reorder_trace_host_async(hcc_pipeline *p, const hcc_bvh *bvh
  * fill each other's gaps: up to 2^23 rays in total, b's keys and sort run on a stream of the pipeline's own beside a's (forked from and
  * joined back into `stream` by events), then a's traversal kernel and, as a dependent launch that does not wait
  * for it, b's: b's CTAs become resident as a's run out.  Both batches must be complete in memory when the call
- * is made.  Results are those of two hcc_reorder_trace calls.  Either n may be 0.  The first call allocates a
- * second key buffer and sort workspace.  Per-stage timing is not recorded. */
+ * is made.  Results are those of two hcc_reorder_trace calls.  Either n may be 0.  Needs a pipeline created
+ * with HCC_PIPELINE_PAIR (else HCC_ERR_INVALID_ARG).  Per-stage timing is not recorded. */
 HCC_API int32_t hcc_reorder_trace_pair(hcc_pipeline *p, const hcc_bvh *bvh, const hcc_cut *cut, int32_t order,
                                uint32_t key_bits, const float *rays_a_dev, uint64_t n_a, int32_t mode_a,
                                void *hits_a_dev, const float *rays_b_dev, uint64_t n_b, int32_t mode_b,

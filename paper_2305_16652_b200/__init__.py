@@ -369,12 +369,13 @@ def anc(keys, perm=None, stream=None):
 
 # ---------------------------------------------------------------------------------- pipeline
 class Pipeline:
-    """Per-batch scratch (hcc_pipeline_create) and the one-call path encode -> sort -> trace."""
+    """Per-batch scratch (hcc_pipeline_create) and the one-call path encode -> sort -> trace.  host_staging: scratch for the
+    host-buffer calls; pair: scratch for reorder_trace_pair."""
 
-    def __init__(self, n_max, container_bits_max=64, host_staging=False):
+    def __init__(self, n_max, container_bits_max=64, host_staging=False, pair=False):
         self._h = _vp()
         self.n_max = int(n_max)
-        _check(lib().hcc_pipeline_create(self.n_max, int(container_bits_max), 1 if host_staging else 0,
+        _check(lib().hcc_pipeline_create(self.n_max, int(container_bits_max), (1 if host_staging else 0) | (2 if pair else 0),
                                          ctypes.byref(self._h)))
 
     def set_sort_skip_bits(self, bits):

@@ -12,7 +12,7 @@ struct hcc_pipeline {
     uint32_t container_bits_max;
     bool host_staging;
     void *d_keys;
-    uint32_t *d_perm[2];   // alternate per call: a call's sort may run while the previous call's trace still reads its perm
+    uint32_t *d_perm[2];   // one per batch of a pair call (single calls use the first)
     uint32_t calls;        // calls made
     cudaStream_t last_stream;
     bool timing;           // record the per-stage events (hcc_pipeline_set_timing)
@@ -73,9 +73,10 @@ extern "C" int32_t hcc_pipeline_destroy(hcc_pipeline *p) {
     return HCC_OK;
 }
 
-extern "C" int32_t hcc_pipeline_create(uint64_t n_max, uint32_t container_bits_max, uint32_t host_staging,
+extern "C" int32_t hcc_pipeline_create(uint64_t n_max, uint32_t container_bits_max, uint32_t flags,
                                        hcc_pipeline **out) {
     HCC_REQUIRE(out, HCC_ERR_INVALID_ARG, "hcc_pipeline_create: NULL out");
+    HCC_REQUIRE((flags & ~(HCC_PIPELINE_HOST_STAGING | HCC_PIPELINE_PAIR)) == 0, HCC_ERR_INVALID_ARG, "hcc_pipeline_create: unknown flags %u", flags);
     *out = nullptr;
     HCC_REQUIRE(n_max >= 1 && n_max < (1ull << 30), HCC_ERR_INVALID_ARG, "hcc_pipeline_create: n_max must be in 1..2^30-1");
     HCC_REQUIRE(container_bits_max == 32 || container_bits_max == 64, HCC_ERR_INVALID_ARG,
@@ -84,7 +85,8 @@ extern "C" int32_t hcc_pipeline_create(uint64_t n_max, uint32_t container_bits_m
     memset(p, 0, sizeof *p);
     p->n_max = n_max;
     p->container_bits_max = container_bits_max;
-    p->host_staging = host_staging != 0;
+    p->host_staging = (flags & HCC_PIPELINE_HOST_STAGING) != 0;
+    const bool pair = (flags & HCC_PIPELINE_PAIR) != 0;
     int32_t rc = hcc_sort_workspace_bytes(n_max, container_bits_max, &p->ws_bytes);
     if (rc != HCC_OK) { delete p; return rc; }
     cudaError_t e = cudaMalloc(&p->d_keys, (size_t)(container_bits_max / 8) * n_max);
@@ -93,6 +95,12 @@ extern "C" int32_t hcc_pipeline_create(uint64_t n_max, uint32_t container_bits_m
     if (e == cudaSuccess) e = cudaMalloc(&p->d_ws, p->ws_bytes);
     if (e == cudaSuccess && p->host_staging) e = cudaMalloc((void **)&p->d_rays, 32 * n_max);
     if (e == cudaSuccess && p->host_staging) e = cudaMalloc(&p->d_hits, 16 * n_max);
+    // hcc_reorder_trace_pair: the second batch's keys and sort workspace, the side stream and its fork / join events
+    if (e == cudaSuccess && pair) e = cudaMalloc(&p->d_keys2, (size_t)(container_bits_max / 8) * n_max);
+    if (e == cudaSuccess && pair) e = cudaMalloc(&p->d_ws2, p->ws_bytes);
+    if (e == cudaSuccess && pair) e = cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess && pair) e = cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
+    if (e == cudaSuccess && pair) e = cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking);
     for (int i = 0; i < 6 && e == cudaSuccess; ++i) e = cudaEventCreate(&p->ev[i]);
     if (e != cudaSuccess) {
         set_error("hcc_pipeline_create: %s", cudaGetErrorString(e));
@@ -191,20 +199,6 @@ extern "C" int32_t hcc_reorder_trace(hcc_pipeline *p, const hcc_bvh *bvh, const 
     return HCC_OK;
 }
 
-static int32_t ensure_side(hcc_pipeline *p) {
-    if (p->side) return HCC_OK;
-    cudaError_t e = cudaMalloc(&p->d_keys2, (size_t)(p->container_bits_max / 8) * p->n_max);
-    if (e == cudaSuccess) e = cudaMalloc(&p->d_ws2, p->ws_bytes);
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
-    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking);
-    if (e != cudaSuccess) {
-        set_error("hcc_reorder_trace_pair: %s", cudaGetErrorString(e));
-        return e == cudaErrorMemoryAllocation ? HCC_ERR_OUT_OF_MEMORY : HCC_ERR_CUDA;
-    }
-    return HCC_OK;
-}
-
 // Both batches of one bounce in one call (PAPER.md:245-247 runs the three kernels per batch; a renderer has the diffuse
 // and the shadow batch of a bounce at the same time).  Schedule:
 //   stream s    : keys + sort of batch a  --+--> trace a --> trace b (dependent launch that does NOT wait for trace a)
@@ -223,8 +217,8 @@ extern "C" int32_t hcc_reorder_trace_pair(hcc_pipeline *p, const hcc_bvh *bvh, c
     BatchPlan pa, pb;
     int32_t rc = plan_batch(p, cut, order, key_bits, n_a, mode_a, &pa);
     if (rc == HCC_OK) rc = plan_batch(p, cut, order, key_bits, n_b, mode_b, &pb);
-    if (rc == HCC_OK) rc = ensure_side(p);
     if (rc != HCC_OK) return rc;
+    HCC_REQUIRE(p->side, HCC_ERR_INVALID_ARG, "hcc_reorder_trace_pair: pipeline created without HCC_PIPELINE_PAIR");
     uint32_t *slot_a = nullptr, *slot_b = nullptr;
     // side by side only while the key and sort kernels are latency-bound (a few million rays): large batches fill the
     // machine on their own and two sorts at once only get in each other's way (config 3: +1-12 % when run side by side)

@@ -38,7 +38,7 @@ def _run(hcc, name, bounce, res_scale=1.0):
     ent, cnt = cut.read()
     assert np.array_equal(ent, tables.entry_node) and np.array_equal(cnt, tables.table_cnt)
     info = cut.info()
-    pipe = hcc.Pipeline(shadow.shape[0], 64)
+    pipe = hcc.Pipeline(shadow.shape[0], 64, pair=True)
     kept = []
     for rays_h, mode in ((diffuse, hcc.TRACE_CLOSEST), (shadow, hcc.TRACE_ANY)):
         n = rays_h.shape[0]

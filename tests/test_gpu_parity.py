@@ -357,7 +357,10 @@ def test_pipeline_pair_matches_two_calls(hcc, dev_cases, name, K, bits):
     d = dev_cases[name]
     cut = hcc.select_cut(d["bvh"], hcc.density(d["bvh"]), K, bits)
     ra, rb = d["diffuse"], d["shadow"]
-    pipe = hcc.Pipeline(max(ra.shape[0], rb.shape[0]), 64)
+    pipe = hcc.Pipeline(max(ra.shape[0], rb.shape[0]), 64, pair=True)
+    with pytest.raises(hcc.HccError):      # a pipeline without the pair scratch refuses the call
+        hcc.Pipeline(16, 64).reorder_trace_pair(d["bvh"], cut, hcc.ORDER_HCC, ra[:8], hcc.TRACE_CLOSEST, torch.empty((8, 4), device="cuda"),
+                                                rb[:8], hcc.TRACE_ANY, torch.empty(8, dtype=torch.uint8, device="cuda"), key_bits=bits)
     ref_a = hcc.trace(d["bvh"], ra, None, hcc.TRACE_CLOSEST)
     ref_b = hcc.trace(d["bvh"], rb, None, hcc.TRACE_ANY)
     ha, hb = torch.empty_like(ref_a), torch.empty_like(ref_b)
