@@ -89,6 +89,9 @@ constexpr int ENC_THREADS = 256;
 // dependent fp32 operations on the half-rate min/max pipe), so the staged tables are shared by as many threads as
 // possible: two CTAs of 768 threads at <= 40 registers (48 warps per SM) while two copies of the tables fit, else one
 // CTA of 1024 threads.
+#ifndef HCC_ENC_STAGE_BYTES           // whole levels of the cut are staged in shared memory, top down, while they fit this
+#define HCC_ENC_STAGE_BYTES (160 * 1024)
+#endif
 #ifndef HCC_ENC_WIDE_THREADS
 #define HCC_ENC_WIDE_THREADS 768
 #define HCC_ENC_WIDE_CTAS 2
@@ -106,7 +109,14 @@ k_encode_hcc(const float4 *__restrict__ rays, uint64_t n, const CutDev cut, uint
     const ulonglong2 *g_box = reinterpret_cast<const ulonglong2 *>(cut.boxes);
     if (wait) pdl_wait();
     pdl_trigger();
-    for (uint32_t i = threadIdx.x; i < 2u * smem_entries; i += blockDim.x) s_box[i] = g_box[i];
+    // staged tables are padded by one 16-byte unit each: the tables of a level are a power-of-two number of bytes apart,
+    // so without the pad the lanes of a warp that read DIFFERENT tables (levels below the first) would all hit the same banks
+    for (uint32_t i = threadIdx.x; i < 2u * smem_entries; i += blockDim.x) {
+        const uint32_t e = i >> 1;
+        uint32_t l = 0;
+        while (l + 1 < cut.m && e >= cut.ent_off[l + 1]) ++l;
+        s_box[i + cut.tab_off[l] + (e - cut.ent_off[l]) / cut.w[l]] = g_box[i];
+    }
     __syncthreads();
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     for (uint64_t ri = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; ri < n; ri += stride) {
@@ -125,7 +135,7 @@ k_encode_hcc(const float4 *__restrict__ rays, uint64_t n, const CutDev cut, uint
             if (alive) {
                 const uint32_t e0 = cut.ent_off[l] + table * w;
                 const bool in_smem = e0 < smem_entries;           // uniform per level
-                const ulonglong2 *box = in_smem ? s_box + 2 * (size_t)e0 : g_box + 2 * (size_t)e0;
+                const ulonglong2 *box = in_smem ? s_box + 2 * (size_t)e0 + (cut.tab_off[l] + table) : g_box + 2 * (size_t)e0;
                 const uint32_t cnt = (uint32_t)(in_smem ? box[1].y : ldg_u2(box + 1).y);   // low word = count
                 // entries [0,cnt) are valid; entry j -> bit (w-1-j)
                 uint32_t c_hi = cnt > 32u ? cnt - 32u : 0u;       // only flat tables wider than 32
@@ -289,13 +299,15 @@ int32_t hcc::encode_launch(const float *rays_dev, uint64_t n, const hcc_cut *cut
     HCC_REQUIRE(n < (1ull << 32), HCC_ERR_UNSUPPORTED, "hcc_encode: n >= 2^32");
     const CutDev &d = cut->dev;
     // stage whole levels, top down, while they fit in 160 KB (leaves room for 1 CTA/SM at worst)
-    const size_t budget = 160 * 1024;
+    const size_t budget = HCC_ENC_STAGE_BYTES;
     uint32_t smem_entries = 0;
+    uint32_t smem_tables = 0;
     for (uint32_t l = 0; l < d.m; ++l) {
         uint32_t end = d.ent_off[l] + d.n_tab[l] * d.w[l];
-        if ((size_t)end * 32 <= budget) smem_entries = end; else break;
+        if ((size_t)end * 32 + (size_t)(d.tab_off[l] + d.n_tab[l]) * 16 <= budget) { smem_entries = end; smem_tables = d.tab_off[l] + d.n_tab[l]; }
+        else break;
     }
-    size_t smem = (size_t)smem_entries * 32;
+    size_t smem = (size_t)smem_entries * 32 + (size_t)smem_tables * 16;     // one 16-byte pad per staged table (bank spread)
     const bool wide = ENC_WIDE_CTAS * (smem + 1024) <= 200 * 1024;     // two CTAs' tables (+ the per-CTA reserve) fit one SM
     if (cut->container_bits == 32) {
         HCC_CUDA_TRY(encode_attr<uint32_t>(budget));
