@@ -42,7 +42,8 @@ UNIT = "Mrays/s"
 #  encode: 32 B ray read + key write;  sort: one histogram read + per pass read+write of (key, id)
 #  trace : lane-operations = 68 per wide-node record fetched (four quantised child boxes: 24 cell->float
 #          conversions, 24 fma, 16 min/max, 4 compares, trace.cu) + 36 per triangle test (the formula in
-#          include/hcc.h); encode: 26 per exact fp32 slab test (6 sub, 6 mul, 12 min/max, compare, bit).
+#          include/hcc.h); encode: 26 per exact fp32 slab test AS DEFINED (6 sub, 6 mul, 12 min/max, compare, bit); the kernel's
+#          oriented form of the test executes 20 of them (no per-axis min/max), so alu_frac is algorithmic work over peak.
 OPS_BOX, OPS_NODE, OPS_TRI = 26, 68, 36
 # the same operations weighted by the issue cycles their pipe takes (B300_MICROARCH.md: min/max, compare, select, PRMT run on the
 # ALU pipe at 16 lanes per scheduler and clock = 2 cycles per warp instruction; fma/mul/add at 1): per wide record 44 ALU-pipe

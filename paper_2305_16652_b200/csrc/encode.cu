@@ -84,48 +84,113 @@ __device__ __forceinline__ uint32_t table_mask(const RayEnc &r, const ulonglong2
     return mask;
 }
 
+// ---- staged (shared-memory) tables: the oriented form of the same test.
+// A staged entry is three 16-byte units, one per axis a: {lo_a, hi_a, -hi_a, -lo_a}.  A ray that moves in +a reads the pair at
+// byte 0 and keeps its origin; one that moves in -a reads the pair at byte 8 and negates its origin and reciprocal.  Either
+// way (pair - o') * |inv| is (t_near, t_far) of that axis in this order, BIT FOR BIT the t1 / t2 of slab_hit (negating both
+// operands of a subtraction or one of a multiplication negates the rounded result), so the six per-axis min/max disappear:
+// tn = max(tmin, max_a t_near), tf = min(tmax, min_a t_far).  Only a ray with a zero (or NaN) direction component can
+// tell the two forms apart (0 * inf = NaN is dropped by min/max but would be SELECTED here): those rays take slab_hit.
+struct RayOri {
+    f32x2 ox, oy, oz, ix, iy, iz;   // (o'_a, o'_a), (|inv_a|, |inv_a|)
+    uint32_t bx, by, bz;            // byte offset of the axis pair inside an entry: 16 * a + (8 if the ray moves in -a)
+};
+
+__device__ __forceinline__ f32x2 lds_pair(uint32_t addr) {
+    f32x2 v;
+    asm volatile("ld.shared.b64 %0, [%1];" : "=l"(v) : "r"(addr));
+    return v;
+}
+
+// Mask of one staged table over entries [j0, j1): entry j -> bit (j1-1-j).  ent = shared-window address of entry 0.
+__device__ __forceinline__ uint32_t staged_mask(const RayOri &q, float tmin, float tmax, uint32_t ent, uint32_t j0, uint32_t j1) {
+    uint32_t mask = 0;
+#pragma unroll 4
+    for (uint32_t j = j0; j < j1; ++j) {
+        const uint32_t e = ent + 48u * j;
+        float nx, fx, ny, fy, nz, fz;
+        unpack2(mul2(sub2(lds_pair(e + q.bx), q.ox), q.ix), nx, fx);
+        unpack2(mul2(sub2(lds_pair(e + q.by), q.oy), q.iy), ny, fy);
+        unpack2(mul2(sub2(lds_pair(e + q.bz), q.oz), q.iz), nz, fz);
+        const float tn = fmaxf(max3(nx, ny, nz), tmin);
+        const float tf = fminf(min3(fx, fy, fz), tmax);
+        mask = (mask << 1) | (tn <= tf ? 1u : 0u);
+    }
+    return mask;
+}
+
+// The same table for a ray with a zero or NaN direction component: slab_hit on the (lo, hi) pairs of the staged entries.
+__device__ __forceinline__ uint32_t staged_mask_generic(const RayEnc &r, uint32_t ent, uint32_t j0, uint32_t j1) {
+    uint32_t mask = 0;
+    for (uint32_t j = j0; j < j1; ++j) {
+        const uint32_t e = ent + 48u * j;
+        float lx, hx, ly, hy, lz, hz;
+        unpack2(lds_pair(e), lx, hx);
+        unpack2(lds_pair(e + 16u), ly, hy);
+        unpack2(lds_pair(e + 32u), lz, hz);
+        ulonglong2 A;
+        A.x = pack2(lx, ly); A.y = pack2(hx, hy);
+        mask = (mask << 1) | (slab_hit(r, A, pack2(lz, hz)) ? 1u : 0u);
+    }
+    return mask;
+}
+
 constexpr int ENC_THREADS = 256;
-// The HCC encoder's CTA shapes: its speed is set by how many warps an SM holds (the slab tests are chains of
-// dependent fp32 operations on the half-rate min/max pipe), so the staged tables are shared by as many threads as
-// possible: two CTAs of 768 threads at <= 40 registers (48 warps per SM) while two copies of the tables fit, else one
-// CTA of 1024 threads.
+// The HCC encoder runs one CTA of 1,024 threads per SM (64 registers, 32 warps): with the oriented tables below the kernel
+// keeps two forms of the ray in registers, and 64 registers without spills beat more warps at 40 (two CTAs of 768: +14 %).
 #ifndef HCC_ENC_STAGE_BYTES           // whole levels of the cut are staged in shared memory, top down, while they fit this
 #define HCC_ENC_STAGE_BYTES (160 * 1024)
 #endif
-#ifndef HCC_ENC_WIDE_THREADS
-#define HCC_ENC_WIDE_THREADS 768
-#define HCC_ENC_WIDE_CTAS 2
-#endif
-constexpr int ENC_WIDE_THREADS = HCC_ENC_WIDE_THREADS, ENC_WIDE_CTAS = HCC_ENC_WIDE_CTAS, ENC_MAX_THREADS = 1024;
+constexpr int ENC_HCC_THREADS = 1024;
 
 // Alg. 1: line 1 "copy cut nodes from global memory into shared memory" (the first
 // smem_entries entries = whole levels), line 2 grid-stride "while have ray", lines 4-6 per
 // level.  One ray per thread per iteration; 32-byte rays read as two 16-byte loads.
-template <typename KeyT, int THREADS, int MIN_CTAS>
-__global__ void __launch_bounds__(THREADS, MIN_CTAS)
+template <typename KeyT>
+__global__ void __launch_bounds__(ENC_HCC_THREADS, 1)
 k_encode_hcc(const float4 *__restrict__ rays, uint64_t n, const CutDev cut, uint32_t smem_entries,
              KeyT *__restrict__ keys, int wait) {
     extern __shared__ ulonglong2 s_box[];
     const ulonglong2 *g_box = reinterpret_cast<const ulonglong2 *>(cut.boxes);
     if (wait) pdl_wait();
     pdl_trigger();
-    // staged tables are padded by one 16-byte unit each: the tables of a level are a power-of-two number of bytes apart,
-    // so without the pad the lanes of a warp that read DIFFERENT tables (levels below the first) would all hit the same banks
-    for (uint32_t i = threadIdx.x; i < 2u * smem_entries; i += blockDim.x) {
-        const uint32_t e = i >> 1;
+    // staging: entry e of table T (numbered over all levels) goes to 16-byte units 3 * e + T + 1 .. + 3 in the oriented form;
+    // unit 3 * (first entry of T) + T holds the table's entry count.  The extra unit per table also spreads the tables over
+    // the banks (without it the tables of a level are a power-of-two number of bytes apart and lanes that read different
+    // tables would all hit the same banks).
+    float4 *s_unit = reinterpret_cast<float4 *>(s_box);
+    for (uint32_t e = threadIdx.x; e < smem_entries; e += blockDim.x) {
         uint32_t l = 0;
         while (l + 1 < cut.m && e >= cut.ent_off[l + 1]) ++l;
-        s_box[i + cut.tab_off[l] + (e - cut.ent_off[l]) / cut.w[l]] = g_box[i];
+        const uint32_t in_level = e - cut.ent_off[l], T = cut.tab_off[l] + in_level / cut.w[l];
+        const float4 A = cut.boxes[2 * (size_t)e], B = cut.boxes[2 * (size_t)e + 1];     // lo.x lo.y hi.x hi.y | lo.z hi.z cnt -
+        float4 *u = s_unit + 3 * (size_t)e + T;
+        if (in_level % cut.w[l] == 0) u[0] = make_float4(B.z, 0.f, 0.f, 0.f);      // the count (a bit pattern)
+        u[1] = make_float4(A.x, A.z, -A.z, -A.x);
+        u[2] = make_float4(A.y, A.w, -A.w, -A.y);
+        u[3] = make_float4(B.x, B.y, -B.y, -B.x);
     }
+    const uint32_t sa_box = (uint32_t)__cvta_generic_to_shared(s_box);
     __syncthreads();
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     for (uint64_t ri = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; ri < n; ri += stride) {
         float4 a, b;
         ld_ray(rays + 2 * ri, a, b);
         RayEnc r;
-        const float iz = 1.0f / b.z;
+        const float ix = 1.0f / b.x, iy = 1.0f / b.y, iz = 1.0f / b.z;
         r.oxy = pack2(a.x, a.y); r.ozz = pack2(a.z, a.z); r.tmin = a.w;
-        r.ixy = pack2(1.0f / b.x, 1.0f / b.y); r.izz = pack2(iz, iz); r.tmax = b.w;
+        r.ixy = pack2(ix, iy); r.izz = pack2(iz, iz); r.tmax = b.w;
+        // the oriented form for the staged tables; a zero or NaN direction component (|inv| not finite) takes the generic test
+        const bool plain = fabsf(ix) < __int_as_float(0x7f800000) && fabsf(iy) < __int_as_float(0x7f800000) &&
+                           fabsf(iz) < __int_as_float(0x7f800000);
+        RayOri q;
+        {
+            const bool nx = ix < 0.0f, ny = iy < 0.0f, nz = iz < 0.0f;
+            const float ox = nx ? -a.x : a.x, oy = ny ? -a.y : a.y, oz = nz ? -a.z : a.z;
+            q.ox = pack2(ox, ox); q.oy = pack2(oy, oy); q.oz = pack2(oz, oz);
+            q.ix = pack2(fabsf(ix), fabsf(ix)); q.iy = pack2(fabsf(iy), fabsf(iy)); q.iz = pack2(fabsf(iz), fabsf(iz));
+            q.bx = nx ? 8u : 0u; q.by = ny ? 24u : 16u; q.bz = nz ? 40u : 32u;
+        }
         unsigned long long key = 0;
         uint32_t table = 0;
         bool alive = true;
@@ -135,13 +200,27 @@ k_encode_hcc(const float4 *__restrict__ rays, uint64_t n, const CutDev cut, uint
             if (alive) {
                 const uint32_t e0 = cut.ent_off[l] + table * w;
                 const bool in_smem = e0 < smem_entries;           // uniform per level
-                const ulonglong2 *box = in_smem ? s_box + 2 * (size_t)e0 + (cut.tab_off[l] + table) : g_box + 2 * (size_t)e0;
-                const uint32_t cnt = (uint32_t)(in_smem ? box[1].y : ldg_u2(box + 1).y);   // low word = count
+                const ulonglong2 *box = g_box + 2 * (size_t)e0;
+                const uint32_t cnt_at = sa_box + 16u * (3u * e0 + cut.tab_off[l] + table), ent = cnt_at + 16u;
+                uint32_t cnt;
+                if (in_smem) asm volatile("ld.shared.u32 %0, [%1];" : "=r"(cnt) : "r"(cnt_at));
+                else cnt = (uint32_t)ldg_u2(box + 1).y;           // low word = count
                 // entries [0,cnt) are valid; entry j -> bit (w-1-j)
                 uint32_t c_hi = cnt > 32u ? cnt - 32u : 0u;       // only flat tables wider than 32
                 unsigned long long m_hi = 0;
-                if (c_hi) m_hi = in_smem ? table_mask<true>(r, box, 0, c_hi) : table_mask<false>(r, box, 0, c_hi);
-                uint32_t m_lo = in_smem ? table_mask<true>(r, box, c_hi, cnt) : table_mask<false>(r, box, c_hi, cnt);
+                uint32_t m_lo;
+                if (in_smem) {
+                    if (plain) {
+                        if (c_hi) m_hi = staged_mask(q, r.tmin, r.tmax, ent, 0, c_hi);
+                        m_lo = staged_mask(q, r.tmin, r.tmax, ent, c_hi, cnt);
+                    } else {
+                        if (c_hi) m_hi = staged_mask_generic(r, ent, 0, c_hi);
+                        m_lo = staged_mask_generic(r, ent, c_hi, cnt);
+                    }
+                } else {
+                    if (c_hi) m_hi = table_mask<false>(r, box, 0, c_hi);
+                    m_lo = table_mask<false>(r, box, c_hi, cnt);
+                }
                 mask = (c_hi ? (m_hi << 32) : 0ull) | (unsigned long long)m_lo;   // cnt bits, entry 0 on top
                 uint32_t rep = (uint32_t)__clzll((long long)mask) - (64u - cnt);  // first hit entry (mask != 0)
                 mask = cnt ? mask << (w - cnt) : 0ull;            // cnt >= 1 keeps the shift below 64
@@ -280,8 +359,7 @@ static cudaError_t encode_attr(size_t budget) {
     static std::atomic<int> done[HCC_MAX_DEVICES];
     const int dev = current_device();
     if (done[dev].load(std::memory_order_acquire)) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(k_encode_hcc<KeyT, ENC_WIDE_THREADS, ENC_WIDE_CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_encode_hcc<KeyT, ENC_MAX_THREADS, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget);
+    cudaError_t e = cudaFuncSetAttribute(k_encode_hcc<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget);
     if (e == cudaSuccess) done[dev].store(1, std::memory_order_release);
     return e;
 }
@@ -304,33 +382,20 @@ int32_t hcc::encode_launch(const float *rays_dev, uint64_t n, const hcc_cut *cut
     uint32_t smem_tables = 0;
     for (uint32_t l = 0; l < d.m; ++l) {
         uint32_t end = d.ent_off[l] + d.n_tab[l] * d.w[l];
-        if ((size_t)end * 32 + (size_t)(d.tab_off[l] + d.n_tab[l]) * 16 <= budget) { smem_entries = end; smem_tables = d.tab_off[l] + d.n_tab[l]; }
+        if ((size_t)end * 48 + (size_t)(d.tab_off[l] + d.n_tab[l]) * 16 <= budget) { smem_entries = end; smem_tables = d.tab_off[l] + d.n_tab[l]; }
         else break;
     }
-    size_t smem = (size_t)smem_entries * 32 + (size_t)smem_tables * 16;     // one 16-byte pad per staged table (bank spread)
-    const bool wide = ENC_WIDE_CTAS * (smem + 1024) <= 200 * 1024;     // two CTAs' tables (+ the per-CTA reserve) fit one SM
+    size_t smem = (size_t)smem_entries * 48 + (size_t)smem_tables * 16;     // oriented entries of 48 bytes + one unit per staged table
     if (cut->container_bits == 32) {
+        auto kern = k_encode_hcc<uint32_t>;
         HCC_CUDA_TRY(encode_attr<uint32_t>(budget));
-        if (wide) {
-            auto kern = k_encode_hcc<uint32_t, ENC_WIDE_THREADS, ENC_WIDE_CTAS>;
-            HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, smem, n, ENC_WIDE_THREADS)), dim3(ENC_WIDE_THREADS), smem, s,
-                                  (const float4 *)rays_dev, n, d, smem_entries, (uint32_t *)keys_dev, kind_waits(kind)));
-        } else {
-            auto kern = k_encode_hcc<uint32_t, ENC_MAX_THREADS, 1>;
-            HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, smem, n, ENC_MAX_THREADS)), dim3(ENC_MAX_THREADS), smem, s,
-                                  (const float4 *)rays_dev, n, d, smem_entries, (uint32_t *)keys_dev, kind_waits(kind)));
-        }
+        HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, smem, n, ENC_HCC_THREADS)), dim3(ENC_HCC_THREADS), smem, s,
+                              (const float4 *)rays_dev, n, d, smem_entries, (uint32_t *)keys_dev, kind_waits(kind)));
     } else {
+        auto kern = k_encode_hcc<unsigned long long>;
         HCC_CUDA_TRY(encode_attr<unsigned long long>(budget));
-        if (wide) {
-            auto kern = k_encode_hcc<unsigned long long, ENC_WIDE_THREADS, ENC_WIDE_CTAS>;
-            HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, smem, n, ENC_WIDE_THREADS)), dim3(ENC_WIDE_THREADS), smem, s,
-                                  (const float4 *)rays_dev, n, d, smem_entries, (unsigned long long *)keys_dev, kind_waits(kind)));
-        } else {
-            auto kern = k_encode_hcc<unsigned long long, ENC_MAX_THREADS, 1>;
-            HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, smem, n, ENC_MAX_THREADS)), dim3(ENC_MAX_THREADS), smem, s,
-                                  (const float4 *)rays_dev, n, d, smem_entries, (unsigned long long *)keys_dev, kind_waits(kind)));
-        }
+        HCC_CUDA_TRY(launch_k(kind, kern, dim3(grid_for((const void *)kern, smem, n, ENC_HCC_THREADS)), dim3(ENC_HCC_THREADS), smem, s,
+                              (const float4 *)rays_dev, n, d, smem_entries, (unsigned long long *)keys_dev, kind_waits(kind)));
     }
     return HCC_OK;
 }
