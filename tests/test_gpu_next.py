@@ -185,3 +185,41 @@ def test_alg3_discard_tables_and_keys_bit_exact(hcc, cases, name, widths, bits):
     assert np.array_equal(ent2, kept.entry_node) and np.array_equal(cnt2, kept.table_cnt)
     with pytest.raises(hcc.HccError):
         hcc.select_cut_levels(d["bvh"], had, widths, bits, flags=6)
+
+
+def test_plain_launches_give_the_same_results():
+    """HCC_NO_PDL=1 turns every chained / overlapping launch into a plain one (the library's A/B switch, read once per
+    process): the pair call and the single calls still agree with the default build's hits, bit for bit."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = r'''
+import sys, hashlib
+sys.path.insert(0, %r)
+import numpy as np, torch, hcc_inputs, oracle
+import paper_2305_16652_b200 as hcc
+w = hcc_inputs.Workload("tiny")
+b = w.bvh
+def tc(bvh, rays):
+    t, p, _, _ = oracle.closest_bvh(rays, bvh.nodes, bvh.prim_idx, bvh.tris); return t, p
+d, s = w.first_bounce(tc)
+bvh = hcc.Bvh(b.nodes, b.tris, b.prim_idx)
+cut = hcc.select_cut(bvh, hcc.density(bvh), w.K, w.key_bits)
+rd, rs = torch.from_numpy(d).cuda(), torch.from_numpy(s).cuda()
+pipe = hcc.Pipeline(rs.shape[0], 64, pair=True)
+hd = torch.empty((rd.shape[0], 4), dtype=torch.float32, device="cuda"); hs = torch.empty(rs.shape[0], dtype=torch.uint8, device="cuda")
+for _ in range(3):
+    pipe.reorder_trace_pair(bvh, cut, hcc.ORDER_HCC, rd, hcc.TRACE_CLOSEST, hd, rs, hcc.TRACE_ANY, hs)
+one_d = pipe.reorder_trace(bvh, cut, hcc.ORDER_HCC, rd, hcc.TRACE_CLOSEST)
+one_s = pipe.reorder_trace(bvh, cut, hcc.ORDER_HCC, rs, hcc.TRACE_ANY)
+assert torch.equal(one_d.view(torch.uint8), hd.view(torch.uint8)) and torch.equal(one_s, hs)
+print("DIGEST", hashlib.sha256(hd.cpu().numpy().tobytes() + hs.cpu().numpy().tobytes()).hexdigest())
+''' % root
+    digests = []
+    for no_pdl in ("0", "1"):
+        env = dict(os.environ, HCC_NO_PDL=no_pdl)
+        r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, env=env, timeout=600, cwd=root)
+        assert r.returncode == 0, r.stderr[-2000:]
+        digests.append([l for l in r.stdout.splitlines() if l.startswith("DIGEST")][-1])
+    assert digests[0] == digests[1]
