@@ -246,6 +246,33 @@ HCC_API int32_t hcc_sort(void *keys_dev, uint64_t n, uint32_t container_bits, ui
 HCC_API int32_t hcc_sort_range(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bit_lo, uint32_t bit_hi,
                        uint32_t *perm_dev, void *workspace_dev, uint64_t workspace_bytes, void *stream);
 
+/* hcc_sort for callers that have no way to obtain device memory for a workspace.  Some users of this
+ * library sit where cudaMalloc is off limits: a plug-in running under a host application that owns the
+ * GPU's memory pool and hands the plug-in only its input and output buffers, a real-time render loop that
+ * must not take the driver's allocation lock, a worker started after its parent has already committed all
+ * of HBM.  For them the sort's workspace (the second key / ray-id buffers of the ping-pong, the digit
+ * histograms and the look-back status rows) lives in a fixed array that is part of
+ * the library image itself: every GPU on which the library's kernels are loaded carries
+ * HCC_SORT_STATIC_BYTES (4 MiB) for it until the process exits, whether or not this call is ever used.
+ * That is why the limit is small: n <= HCC_SORT_STATIC_MAX_N (262,144 pairs, either key width); a larger
+ * n returns HCC_ERR_UNSUPPORTED with a message naming the limit, and nothing is enqueued.
+ *
+ * Same result as hcc_sort(keys_dev, n, container_bits, bits_used, perm_dev, <workspace>, .., stream),
+ * bit for bit; keys_dev is clobbered; the caller still owns keys_dev and perm_dev.  The call makes no
+ * cudaMalloc / cudaFree and calls nothing that does.
+ *  - First call on a device: with that device current, the call looks up the array's device address and
+ *    sets the sort kernels' shared-memory attribute (both cached per device).  Make that first call outside
+ *    any stream capture.
+ *  - There is ONE array per device, shared by every call from every thread.  Two hcc_sort_static calls
+ *    whose kernels can overlap on the GPU (different streams without an ordering between them) race on it
+ *    and give garbage; calls on one stream, or ordered by events, are fine.  The array keeps whatever the
+ *    previous call left in it; the first kernel of each call clears the part that has to start at zero
+ *    (histograms, tickets, status rows), so no call depends on an earlier one. */
+#define HCC_SORT_STATIC_MAX_N 262144u
+#define HCC_SORT_STATIC_BYTES 4194304u
+HCC_API int32_t hcc_sort_static(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bits_used,
+                        uint32_t *perm_dev, void *stream);
+
 /* ---- (a4) trace -----------------------------------------------------------------------
  * Rays are traced through perm_dev (perm_dev == NULL: the input order 0, 1, ..., the NoSort
  * order): warps take 32-rank chunks of consecutive ranks, so the rays a warp holds are

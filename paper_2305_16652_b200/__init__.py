@@ -44,6 +44,7 @@ _SIGNATURES = {
     "hcc_encode_twopoint": [_vp, _u64, _vp, _vp, _u32, _vp, _vp],
     "hcc_sort_workspace_bytes": [_u64, _u32, _pu64],
     "hcc_sort": [_vp, _u64, _u32, _u32, _vp, _vp, _u64, _vp],
+    "hcc_sort_static": [_vp, _u64, _u32, _u32, _vp, _vp],
     "hcc_encode_ppc": [_vp, _vp, _u64, _u32, _vp, _vp],
     "hcc_select_grid": [_vp, _vp, _u32, _u32, _vp, _vp],
     "hcc_cut_read_boxes": [_vp, _vp, _vp],
@@ -309,6 +310,22 @@ def sort(keys, bits_used, perm=None, workspace=None, stream=None, bit_lo=0):
     _check(lib().hcc_sort_range(_dev(keys, (torch.int32, torch.int64), "keys"), n, cb, int(bit_lo), int(bits_used),
                                 _dev(perm, (torch.int32,), "perm"), _vp(workspace.data_ptr()), workspace.numel(),
                                 _stream(stream)))
+    return perm
+
+
+SORT_STATIC_MAX_N = 262144
+
+
+def sort_static(keys, bits_used, perm, stream=None):
+    """hcc_sort_static: hcc_sort without a workspace argument, for code that runs where device memory cannot be
+    allocated (a plug-in inside an application that owns the GPU's memory, a render loop that must stay off the
+    driver's allocation lock).  The workspace is a 4 MiB array inside the library, one per GPU, shared by all
+    calls: at most SORT_STATIC_MAX_N pairs, and two calls must not run on the GPU at the same time.  `perm`
+    (int32 CUDA [n]) is the caller's, as are the keys (clobbered): this function creates no tensor."""
+    n = keys.shape[0]
+    cb = 32 if keys.dtype == torch.int32 else 64
+    _check(lib().hcc_sort_static(_dev(keys, (torch.int32, torch.int64), "keys"), n, cb, int(bits_used),
+                                 _dev(perm, (torch.int32,), "perm"), _stream(stream)))
     return perm
 
 

@@ -437,3 +437,52 @@ extern "C" int32_t hcc_sort(void *keys_dev, uint64_t n, uint32_t container_bits,
     HCC_REQUIRE(bits_used <= container_bits, HCC_ERR_INVALID_ARG, "hcc_sort: bits_used > container_bits");
     return hcc_sort_range(keys_dev, n, container_bits, 0u, bits_used, perm_dev, workspace_dev, workspace_bytes, stream);
 }
+
+// ---- hcc_sort_static: the sort for callers that cannot allocate device memory (include/hcc.h) ----------------
+// The workspace is this array.  It is part of the library image: each GPU that loads these kernels holds it
+// until the process exits.  On the host the name `g_sort_static_ws` is only a handle for the runtime, not a
+// device address, so host code never passes it to a kernel: the address comes from cudaGetSymbolAddress, asked
+// once per device with that device current.
+static __device__ __align__(256) unsigned char g_sort_static_ws[HCC_SORT_STATIC_BYTES];
+
+namespace {
+constexpr uint64_t up256(uint64_t x) { return (x + 255u) / 256u * 256u; }
+// hcc_sort_workspace_bytes(HCC_SORT_STATIC_MAX_N, 64) written out as a constant expression (64-bit keys need the most)
+constexpr uint64_t STATIC_TILES = ((uint64_t)HCC_SORT_STATIC_MAX_N + hcc::SORT_TILE - 1) / hcc::SORT_TILE;
+constexpr uint64_t STATIC_NEED = up256(8ull * HCC_SORT_STATIC_MAX_N) + up256(4ull * HCC_SORT_STATIC_MAX_N) + up256(sizeof(hcc::SortCtl)) +
+                                 up256((uint64_t)hcc::MAX_PASSES * (STATIC_TILES + 1) * hcc::RADIX * sizeof(uint32_t)) + 256;
+static_assert(STATIC_NEED <= HCC_SORT_STATIC_BYTES, "HCC_SORT_STATIC_BYTES too small for HCC_SORT_STATIC_MAX_N pairs");
+
+// device address of g_sort_static_ws on the current device (looked up on the first call there, then cached)
+int32_t static_ws(unsigned char **out) {
+    static std::atomic<unsigned char *> cache[HCC_MAX_DEVICES];
+    int dev = -1;
+    HCC_CUDA_TRY(cudaGetDevice(&dev));
+    HCC_REQUIRE(dev >= 0 && dev < HCC_MAX_DEVICES, HCC_ERR_UNSUPPORTED, "hcc_sort_static: device ordinal %d not supported", dev);
+    unsigned char *p = cache[dev].load(std::memory_order_acquire);
+    if (!p) {
+        void *sym = nullptr;
+        HCC_CUDA_TRY(cudaGetSymbolAddress(&sym, g_sort_static_ws));
+        HCC_REQUIRE(sym && aligned(sym, 256), HCC_ERR_CUDA, "hcc_sort_static: no device address for the static workspace");
+        p = static_cast<unsigned char *>(sym);
+        cache[dev].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return HCC_OK;
+}
+}  // namespace
+
+extern "C" int32_t hcc_sort_static(void *keys_dev, uint64_t n, uint32_t container_bits, uint32_t bits_used, uint32_t *perm_dev,
+                                   void *stream) {
+    HCC_REQUIRE(container_bits == 32 || container_bits == 64, HCC_ERR_INVALID_ARG, "hcc_sort_static: container_bits must be 32 or 64");
+    HCC_REQUIRE(bits_used <= container_bits, HCC_ERR_INVALID_ARG, "hcc_sort_static: bits_used > container_bits");
+    HCC_REQUIRE(n <= HCC_SORT_STATIC_MAX_N, HCC_ERR_UNSUPPORTED,
+                "hcc_sort_static: n = %llu exceeds the static workspace's limit of %u pairs (use hcc_sort with a workspace of your own)",
+                (unsigned long long)n, (unsigned)HCC_SORT_STATIC_MAX_N);
+    if (n == 0) return HCC_OK;
+    unsigned char *ws = nullptr;
+    const int32_t rc = static_ws(&ws);
+    if (rc != HCC_OK) return rc;
+    // the same kernels as hcc_sort; k_sort_init, the first of them, zeroes the control region the last call left behind
+    return sort_launch(keys_dev, n, container_bits, 0u, bits_used, perm_dev, ws, HCC_SORT_STATIC_BYTES, (cudaStream_t)stream, nullptr, LK_FIRST);
+}
