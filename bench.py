@@ -108,6 +108,46 @@ def _peaks():
         return 6650.0, 1965.0, "fallback"
 
 
+# ---- the final stdout line.  The driver keeps only the tail of stdout, so the LAST line is one compact JSON object
+# (under 4 KB); everything else (per-order splits, later bounces, other configs, studies, counters) is printed as
+# separate {"section": ...} lines BEFORE it, and only when asked for by flag, or written to --full-json.
+FINAL_KEYS = ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline", "cut")
+FINAL_MAX_BYTES = 4096
+
+
+def _round(x, sig=5):
+    if isinstance(x, float):
+        return float(f"{x:.{sig}g}") if x == x and abs(x) != float("inf") else None
+    if isinstance(x, dict):
+        return {k: _round(v, sig) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_round(v, sig) for v in x]
+    return x
+
+
+def final_line(full):
+    """The compact last line from the full result dict: the contract's keys, the four whole-step speed-ups of the HCC
+    order and ms + roofline fraction per stage and batch."""
+    out = {k: full.get(k) for k in FINAL_KEYS}
+    sp = full.get("speedup_hcc") or {}
+    out["speedup_hcc"] = {k: sp.get(k) for k in ("pair_incl_vs_nosort", "pair_incl_vs_twopoint", "all_incl_vs_nosort", "all_incl_vs_twopoint")}
+    st = full.get("stages_roofline_hcc") or {}
+    out["stages_roofline_hcc"] = {b: {stg: {"ms": v.get("ms"), "bound": v.get("bound"), "frac": v.get("frac")} for stg, v in d.items()}
+                                  for b, d in st.items()}
+    if full.get("strong_scaling"):          # N > 1 only: the strong-scaling leg beside the weak-scaling value
+        out["strong_scaling"] = {k: v for k, v in full["strong_scaling"].items() if k != "how"}
+    line = json.dumps(_round(out), separators=(",", ":"))
+    if len(line) >= FINAL_MAX_BYTES:       # never let a long free-text field cost the round its measurement
+        for k in ("how", "traffic_unit", "peak_source", "sample", "parallelism"):
+            for d in (out.get("e2e"), out.get("roofline"), out.get("cpu_baseline"), out.get("config")):
+                if isinstance(d, dict) and k in d and isinstance(d[k], str):
+                    d[k] = d[k][:60]
+        line = json.dumps(_round(out), separators=(",", ":"))
+    assert len(line) < FINAL_MAX_BYTES, len(line)
+    return line
+
+
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -497,7 +537,8 @@ def run_ours(args):
         sc0 = sc if rank == 0 else load(args.workload, args.res_scale, seed_rank=0)
         if sc0 is not sc:
             set_bounce(sc0, args.bounce)
-        spipe = hcc.Pipeline(max(shard.ray_shard(sc0.n_s, 0, world)[1], 1), 64)
+        shard_len = lambda n_: shard.ray_shard(n_, 0, world)[1] - shard.ray_shard(n_, 0, world)[0]
+        spipe = hcc.Pipeline(max(shard_len(sc0.n_d), shard_len(sc0.n_s), 1), 64)
 
         def sstep():
             return [shard.sharded_reorder_trace(spipe, sc0.bvh, sc0.cut, hcc.ORDER_HCC, rays, mode, rank, world,
@@ -538,12 +579,14 @@ def run_ours(args):
         tr = diag[name]["orders"]["hcc"]["lane_ops"] / (o["trace_ms"] * 1e-3) / 1e12
         enc_ops = nb * info["bits_used"] * OPS_BOX / (o["encode_ms"] * 1e-3) / 1e12
         stages[name] = {
-            "encode": {"bound": "hbm", "achieved": enc_gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": enc_gbs / hbm_gbs,
-                       "alu_achieved_tlaneops": enc_ops, "alu_frac": enc_ops / alu_peak, "box_tests_per_ray": info["bits_used"]},
-            "sort": {"bound": "hbm", "achieved": sort_gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": sort_gbs / hbm_gbs,
+            "encode": {"ms": o["encode_ms"], "bound": "hbm", "achieved": enc_gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": enc_gbs / hbm_gbs,
+                       "alu_achieved_tlaneops": enc_ops, "alu_frac": enc_ops / alu_peak, "box_tests_per_ray": info["bits_used"],
+                       # the same fraction with the op counts of SURVEY.md:604 (20 per test; 14 with 3-input min/max) beside the definition's 26
+                       "alu_frac_by_ops_per_test": {str(k_): enc_ops * k_ / OPS_BOX / alu_peak for k_ in (OPS_BOX, 20, 14)}},
+            "sort": {"ms": o["sort_ms"], "bound": "hbm", "achieved": sort_gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": sort_gbs / hbm_gbs,
                      "passes": passes, "bytes_per_pair_moved": sb_real, "bytes_per_pair_survey": sb_algo,
                      "frac_survey_bytes": nb * sb_algo / (o["sort_ms"] * 1e-3) / 1e9 / hbm_gbs},
-            "trace": {"bound": "alu", "achieved": tr, "peak": alu_peak, "unit": "Tlaneop/s", "frac": tr / alu_peak,
+            "trace": {"ms": o["trace_ms"], "bound": "alu", "achieved": tr, "peak": alu_peak, "unit": "Tlaneop/s", "frac": tr / alu_peak,
                       "frac_pipe_weighted": diag[name]["orders"]["hcc"]["lane_cycles"] / (o["trace_ms"] * 1e-3) / 1e12 / alu_peak}}
     # dominant kernel of the step
     dom = max((("diffuse", "trace"), ("shadow", "trace"), ("diffuse", "sort"), ("shadow", "sort"),
@@ -564,7 +607,7 @@ def run_ours(args):
     by_bounce = {str(args.bounce): {"speedup_hcc": speed, "rays": n,
                                     "trace_ms": {o: {b_: orders[o][b_]["trace_ms"] for b_ in ("diffuse", "shadow")} for o in orders}}}
     shuffled = None
-    if world == 1 and not args.quick:
+    if world == 1 and args.bounces:
         k_b = max(3, min(args.steps, 10))
         for b_i in range(args.bounce + 1, args.bounce + 3):
             set_bounce(sc, b_i)
@@ -598,7 +641,7 @@ def run_ours(args):
         return float(np.median(out))
 
     large = None
-    if world == 1 and not args.no_large_n:
+    if world == 1 and args.large_n:
         reps = max(1, (1 << 25) // n_s)
         big = shadow.repeat(reps, 1) if reps > 1 else shadow
         nb = big.shape[0]
@@ -811,6 +854,7 @@ def run_ours(args):
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
             "config": dict(_config(args, w, n_d, n_s, l2="flushed between timed steps (256 MiB write)", world=world),
+                           lib=os.path.relpath(hcc.LIB_PATH, ROOT), no_pdl=os.environ.get("HCC_NO_PDL") == "1",
                            **({"shared_gpu_code_path_check": True} if shared_gpu else {})),
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
             "roofline": roof, "cpu_baseline": cpu,
@@ -821,7 +865,16 @@ def run_ours(args):
             "strong_scaling": strong, "other_configs": others, "studies": studies,
             "diagnostics": diag,
             "paper_context": "RTX 3060, Breakfast: HCC 67.6 vs NoSort 37.4 vs TwoPoint 56.8 Mrays/s trace-only (PAPER.md:294-299); not comparable"}
-    print(json.dumps(line))
+    if args.full_json:
+        with open(args.full_json, "w") as f:
+            json.dump(line, f)
+    # what the flags asked for beyond the headline: one JSON line per section, BEFORE the final line
+    for name in ("orders", "speedup_hcc", "stages_roofline_hcc", "two_stream_step", "sort_truncated_step", "diagnostics",
+                 "speedup_hcc_by_bounce", "shuffled_input", "stages_roofline_large_batch", "strong_scaling", "other_configs", "studies"):
+        if args.sections and line.get(name) is not None:
+            print(json.dumps({"section": name, "data": _round(line[name], 6)}, separators=(",", ":")))
+    sys.stdout.flush()
+    print(final_line(line))
     if world > 1:
         dist.destroy_process_group()
     return 0
@@ -839,14 +892,19 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--bounce", type=int, default=1, help="which bounce's ray batches to run (1 = rays off the primary hits)")
     ap.add_argument("--res-scale", type=float, default=1.0, help="image scale of the workload (1.0 = the config's resolution)")
-    ap.add_argument("--studies", action="store_true", default=True,
-                    help="the NEXT-row studies: sort truncation, lambda/ANC, grid and PPC orders, config-4 sweep (on by default)")
-    ap.add_argument("--no-studies", dest="studies", action="store_false", help="skip the studies (about 45 s)")
-    ap.add_argument("--no-large-n", action="store_true", help="skip the large-batch encode/sort roofline leg")
-    ap.add_argument("--configs", default="fig1,large", help="comma list of further configs to run at their stated sizes (fig1,large): other_configs")
+    ap.add_argument("--studies", action="store_true",
+                    help="the NEXT-row studies: sort truncation, lambda/ANC, grid and PPC orders, config-4 sweep (about 45 s; off by default)")
+    ap.add_argument("--no-studies", dest="studies", action="store_false", help="(default)")
+    ap.add_argument("--large-n", action="store_true", help="the large-batch (33.5 M rays) encode/sort roofline leg")
+    ap.add_argument("--no-large-n", dest="large_n", action="store_false", help="(default)")
+    ap.add_argument("--configs", default="", help="comma list of further configs to run at their stated sizes (fig1,large): other_configs")
+    ap.add_argument("--bounces", action="store_true", help="the two later bounces and the shuffled-input leg of the workload")
+    ap.add_argument("--full-json", default="", help="write the complete result (every section) to this file")
+    ap.add_argument("--sections", action="store_true",
+                    help="print every section of the result as its own JSON line before the final compact line")
     ap.add_argument("--counters-all", action="store_true", help="per-order trace counters for --configs too")
     ap.add_argument("--e2e-chunk", type=int, default=1 << 19, help="rays per chunk of the host-buffer (e2e) leg")
-    ap.add_argument("--quick", action="store_true", help="skip the later-bounce and shuffled-input legs")
+    ap.add_argument("--quick", action="store_true", help="(default; kept for old command lines) no later-bounce and shuffled-input legs")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

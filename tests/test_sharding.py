@@ -128,7 +128,10 @@ def test_bench_two_ranks_code_path_on_one_gpu():
                         "--no-studies", "--no-cpu-baseline", "--no-large-n", "--quick"], capture_output=True, text=True, env=env,
                        timeout=600, cwd=root)
     assert r.returncode == 0, r.stderr[-2000:]
-    line = json.loads([l for l in r.stdout.splitlines() if l.startswith("{")][-1])
+    last = r.stdout.splitlines()[-1]
+    assert last.startswith("{") and len(last) < 4096       # the driver parses the last line and keeps only stdout's tail
+    line = json.loads(last)
+    assert line["value"] > 0 and line["roofline"]["frac"] > 0 and line["e2e"]["value"] > 0
     assert line["n_gpus"] == 2 and line["config"]["shared_gpu_code_path_check"] is True
     s = line["strong_scaling"]
     assert s["ranks"] == 2 and s["scaling"] == "strong" and s["gathered_hits_equal_unsharded"] is True
