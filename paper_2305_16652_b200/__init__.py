@@ -356,7 +356,7 @@ def keys_to_numpy(keys):
 def trace_stats(bvh, rays, perm=None, mode=TRACE_CLOSEST, stream=None):
     """hcc_trace_stats: dict(nodes, tris, rays, max_stack, node_bytes_per_ray, tri_bytes_per_ray; per warp-level
     node step: distinct node records (records_per_step) and lanes taking part (lanes_per_step); per warp-level
-    triangle round: lanes busy (lanes_per_tri_round))."""
+    triangle round: triangle tests (tri_tests_per_round; a lane can test several triangles of its leaf in one round))."""
     n = rays.shape[0]
     hits = (torch.empty((n, 4), dtype=torch.float32, device="cuda") if mode == TRACE_CLOSEST
             else torch.empty(n, dtype=torch.uint8, device="cuda"))
@@ -369,7 +369,7 @@ def trace_stats(bvh, rays, perm=None, mode=TRACE_CLOSEST, stream=None):
                 node_bytes_per_ray=64.0 * nodes / max(nr, 1), tri_bytes_per_ray=64.0 * tris / max(nr, 1),
                 warp_steps=steps, records_per_step=records / max(steps, 1), lanes_per_step=lanes / max(steps, 1),
                 distinct_node_bytes_per_ray=64.0 * records / max(nr, 1),
-                tri_rounds=rounds, tri_tests_per_round=tris / max(rounds, 1), lanes_per_tri_round=tris / max(rounds, 1))
+                tri_rounds=rounds, tri_tests_per_round=tris / max(rounds, 1))
 
 
 def anc(keys, perm=None, stream=None):

@@ -181,6 +181,7 @@ extern "C" int32_t hcc_reorder_trace(hcc_pipeline *p, const hcc_bvh *bvh, const 
     HCC_REQUIRE(p && bvh, HCC_ERR_INVALID_ARG, "hcc_reorder_trace: NULL handle");
     cudaStream_t s = (cudaStream_t)stream;
     p->timed = false;
+    p->host_pending = false;     // hcc_pipeline_synchronize waits for THIS call now (the host form sets it again afterwards)
     BatchPlan pl;
     int32_t rc = plan_batch(p, cut, order, key_bits, n, mode, &pl);
     if (rc != HCC_OK) return rc;
@@ -214,6 +215,7 @@ extern "C" int32_t hcc_reorder_trace_pair(hcc_pipeline *p, const hcc_bvh *bvh, c
     HCC_REQUIRE(p && bvh, HCC_ERR_INVALID_ARG, "hcc_reorder_trace_pair: NULL handle");
     cudaStream_t s = (cudaStream_t)stream;
     p->timed = false;
+    p->host_pending = false;
     BatchPlan pa, pb;
     int32_t rc = plan_batch(p, cut, order, key_bits, n_a, mode_a, &pa);
     if (rc == HCC_OK) rc = plan_batch(p, cut, order, key_bits, n_b, mode_b, &pb);
@@ -290,6 +292,7 @@ extern "C" int32_t hcc_reorder_trace_host(hcc_pipeline *p, const hcc_bvh *bvh, c
     int32_t rc = hcc_reorder_trace_host_async(p, bvh, cut, order, key_bits, rays_host, n, mode, hits_host, stream);
     if (rc != HCC_OK || n == 0) return rc;
     HCC_CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+    p->host_pending = false;
     return HCC_OK;
 }
 

@@ -184,7 +184,8 @@ struct TraceScene {
 // triangle records fetched (64 bytes each): stats[0], stats[1]; stats[2] = rays, stats[3] =
 // deepest stack seen; stats[4] = distinct node records summed over warp-level node steps (what
 // a coherent warp saves), stats[5] = warp-level node steps, stats[6] = lanes taking part in
-// them, stats[7] = warp-level triangle rounds (stats[1] / stats[7] = lanes busy per round).
+// them, stats[7] = warp-level triangle rounds (stats[1] / stats[7] = triangle tests per round; a lane may test
+// several triangles of its leaf in one round, so this can exceed 32).
 // Used for the diagnostics only, never timed.
 template <bool ANY, bool STATS>
 __global__ void __launch_bounds__(TRACE_THREADS, ANY ? TRACE_BLOCKS_PER_SM_ANY : TRACE_BLOCKS_PER_SM)
@@ -485,6 +486,12 @@ k_trace(const TraceScene sc, const float4 *__restrict__ rays, const uint32_t *__
             }
         }
     }
+    // A dependent launch that skipped the wait at entry (hcc_reorder_trace_pair's second traversal kernel) waits HERE, once
+    // its own work is done: a dependent grid has to execute griddepcontrol.wait, and with it this grid cannot complete - and
+    // nothing enqueued behind it on the stream can start - before the first batch's traversal kernel has completed and its
+    // hits are visible.  The CTA only idles until then; every CTA of the primary grid is resident from the start (the grid
+    // is capped at the resident CTAs), so a waiting CTA never stands in the way of one the primary still needs.
+    if (!sc.wait) pdl_wait();
 #ifdef HCC_TRACE_TIMELINE
     if (stats && lane == 0) {
         unsigned long long tl_t1;

@@ -1,6 +1,6 @@
 """Parity at BASELINE.json's full sizes, through the call bench.py times (hcc_reorder_trace on whole
 batches, then both at once through hcc_reorder_trace_pair): config 2 in full (1,048,576 + 2,097,152 rays), config 3 in
-full (16.6 M + 33.2 M rays) and config 5 in full (33.2 M + 66.4 M rays).
+full (16.6 M + 33.2 M rays; bounces 2 and 3) and config 5 in full (33.2 M + 66.4 M rays; bounces 1 and 2).
 The oracle cannot run these batches whole, so: keys and hits of a seeded SAMPLE of rays are compared
 with the oracle one by one (bit-exact keys, hits within the north_star's bars), and the permutation
 is checked by the properties that define it at any size (a permutation; keys non-decreasing along
@@ -16,7 +16,9 @@ torch = pytest.importorskip("torch")
 SAMPLE = 4096
 
 
-def _run(hcc, name, bounce, res_scale=1.0):
+def _run(hcc, name, bounces, res_scale=1.0):
+    """Checks the batches of every bounce in `bounces` (ascending) of one workload; the scene, BVH and cut are built once.
+    Returns {bounce: (diffuse rays, shadow rays)}."""
     import hcc_inputs
     import oracle
     from hcc_inputs import rng as hrng
@@ -27,10 +29,6 @@ def _run(hcc, name, bounce, res_scale=1.0):
     def gpu_trace(_b, rays):
         t, p, _, _ = hcc.hits_to_numpy(hcc.trace(bvh, torch.from_numpy(rays).cuda(), None, hcc.TRACE_CLOSEST))
         return t, p
-    diffuse, shadow = w.first_bounce(gpu_trace)
-    for b_i in range(2, bounce + 1):
-        t, p = gpu_trace(None, diffuse)
-        diffuse, shadow, _ = w.bounce(b_i, diffuse, t, p)
     had = hcc.density(bvh)
     assert np.array_equal(had.cpu().numpy().view(np.uint32), oracle.had(b.nodes).view(np.uint32))
     cut = hcc.select_cut(bvh, had, w.K, w.key_bits)
@@ -38,7 +36,22 @@ def _run(hcc, name, bounce, res_scale=1.0):
     ent, cnt = cut.read()
     assert np.array_equal(ent, tables.entry_node) and np.array_equal(cnt, tables.table_cnt)
     info = cut.info()
-    pipe = hcc.Pipeline(shadow.shape[0], 64, pair=True)
+    diffuse, shadow = w.first_bounce(gpu_trace)
+    pipe = hcc.Pipeline(shadow.shape[0], 64, pair=True)      # later bounces never hold more rays than the first
+    sizes = {}
+    for b_i in range(1, max(bounces) + 1):
+        if b_i > 1:
+            t, p = gpu_trace(None, diffuse)
+            diffuse, shadow, _ = w.bounce(b_i, diffuse, t, p)
+        if b_i in bounces:
+            _check_bounce(hcc, w, b, bvh, cut, tables, info, pipe, diffuse, shadow)
+            sizes[b_i] = (diffuse.shape[0], shadow.shape[0])
+    return sizes
+
+
+def _check_bounce(hcc, w, b, bvh, cut, tables, info, pipe, diffuse, shadow):
+    import oracle
+    from hcc_inputs import rng as hrng
     kept = []
     for rays_h, mode in ((diffuse, hcc.TRACE_CLOSEST), (shadow, hcc.TRACE_ANY)):
         n = rays_h.shape[0]
@@ -83,7 +96,6 @@ def _run(hcc, name, bounce, res_scale=1.0):
     pa, pb = torch.empty_like(ha), torch.empty_like(hb)
     pipe.reorder_trace_pair(bvh, cut, hcc.ORDER_HCC, ra, ma, pa, rb, mb, pb, key_bits=w.key_bits)
     assert torch.equal(pa.view(torch.uint8), ha.view(torch.uint8)) and torch.equal(pb, hb)
-    return diffuse.shape[0], shadow.shape[0]
 
 
 @pytest.fixture(scope="module")
@@ -95,19 +107,24 @@ def hcc():
 
 
 def test_config2_full_size(hcc):
-    n_d, n_s = _run(hcc, "room", 1)
+    n_d, n_s = _run(hcc, "room", [1])[1]
     assert n_d == 1048576 and n_s == 2097152
 
 
-def test_config3_full_size_second_bounce(hcc):
-    """Config 3 (~1 M triangles, 1920x1080x8 spp, 64-bit keys 16x16x16), the rays of bounce 2."""
-    n_d, n_s = _run(hcc, "fig1", 2)
+def test_config3_full_size_second_and_third_bounce(hcc):
+    """Config 3 (~1 M triangles, 1920x1080x8 spp, 64-bit keys 16x16x16; BASELINE.json: 3 bounces): the rays of bounces 2
+    and 3, the incoherent regime the paper's claim is about."""
+    sizes = _run(hcc, "fig1", [2, 3])
+    n_d, n_s = sizes[2]
     assert n_d > 16_000_000 and n_s > 32_000_000
+    assert 4_000_000 < sizes[3][0] <= n_d and sizes[3][1] >= sizes[3][0]
 
 
 def test_config5_full_size(hcc):
     """Config 5 at its stated size: 10.8 M triangles, 7.1 M nodes (a BVH far larger than L2, traversal stacks deeper
     than the shared-memory rows), 1920x1080x16 primaries -> 33.2 M diffuse + 66.4 M shadow rays: K = 16,384, 64-bit
     keys 16x16x8x8."""
-    n_d, n_s = _run(hcc, "large", 1)
+    sizes = _run(hcc, "large", [1, 2])
+    n_d, n_s = sizes[1]
     assert n_d > 33_000_000 and n_s == 2 * n_d
+    assert 8_000_000 < sizes[2][0] <= n_d and sizes[2][1] >= sizes[2][0]      # bounce 2 of BASELINE.json's "4 bounces"

@@ -110,8 +110,10 @@ def test_select_cut_flat_any_K(hcc, dev_cases, name):
 # ------------------------------------------------------------------------------- (a2)
 # (4096, 24) and (65536, 32) are six and eight levels of 4 (the hierarchies bench.py --studies sweeps); (16384, 48)
 # and (65536, 64) have level tables past the 160 KB that fit shared memory (the global-memory branch of the encoder)
+# (256, 32) and (1024, 64) are the paper's own two compressed encoders, MLHCC32 = 16 x 16 and MLHCC64 = 32 x 32
+# (tests/golden/level_widths.txt)
 ENC_REQUESTS = [(64, 32), (32, 32), (64, 64), (1024, 32), (4096, 64), (16384, 64), (256, 16), (48, 48), (1000, 48),
-                (4096, 24), (65536, 32), (16384, 48), (65536, 64)]
+                (4096, 24), (65536, 32), (16384, 48), (65536, 64), (256, 32), (1024, 64)]
 
 
 @pytest.mark.parametrize("name", ["tiny", "room_mid"])
@@ -523,7 +525,8 @@ def test_trace_flat_scene_vs_brute_force(hcc):
 
 
 def test_trace_root_leaf_bvh(hcc):
-    """A BVH that is one leaf (<= 4 triangles): the traversal starts on a leaf reference."""
+    """A BVH that is one leaf (<= 4 triangles): the leaf is wrapped in a wide node of its own (bvh.cu), so the traversal
+    starts on a wide-node reference whose only child is the leaf."""
     import hcc_inputs
     tris = np.array([[[0, 0, 0], [1, 0, 0], [0, 1, 0]], [[0, 0, 0.5], [1, 0, 0.5], [0, 1, 0.5]]], dtype=np.float32)
     b = hcc_inputs.build_bvh(tris)
@@ -531,6 +534,92 @@ def test_trace_root_leaf_bvh(hcc):
     rays = _rand_rays(257, 0x1EAF)
     rays[:, 0:3] = (0.2, 0.2, 1.0)
     _check_trace_both_modes(hcc, b, rays)
+
+
+@pytest.mark.parametrize("scene", ["tiny", "room_small"])
+def test_trace_leaves_of_up_to_eight_triangles(hcc, scene, tiny, room_small):
+    """BVHs built with max_leaf = 8 (include/hcc.h admits leaf counts 1..8): a leaf of 5..8 triangles becomes a wide node
+    of its own with two halves (bvh.cu), which no max_leaf = 4 tree exercises."""
+    import hcc_inputs
+    src = {"tiny": tiny, "room_small": room_small}[scene].bvh
+    b = hcc_inputs.build_bvh(src.tris, max_leaf=8)
+    counts = b.nodes["count"][b.nodes["count"] > 0]
+    assert counts.max() > 4 and counts.max() <= 8
+    lo, hi = b.nodes["lo"][0], b.nodes["hi"][0]
+    rays = _rand_rays(20000 + 11, 0x8EAF)
+    rays[:, 0:3] = lo + (hi - lo) * rays[:, 0:3]         # origins in and around the scene box
+    want = _check_trace_both_modes(hcc, b, rays)
+    assert (~np.isinf(want[0])).sum() > 1000
+
+
+@pytest.mark.parametrize("n_tris", [5, 8])
+def test_trace_single_leaf_of_five_and_eight_triangles_with_ties(hcc, n_tris):
+    """A hand-made BVH that is ONE leaf of 5 or 8 triangles (the root leaf is split into two halves under a wide node).
+    Triangles 1 and n_tris-1 are the same triangle, one in each half: the two tests give the same t, and the lowest
+    prim id must win (include/hcc.h: "ties to the lowest prim id")."""
+    import hcc_inputs
+    import oracle
+    base = np.array([[0.0, 0.0, 0.0], [1.0, 0.0, 0.0], [0.0, 1.0, 0.0]], dtype=np.float32)
+    tris = np.stack([base + np.float32([0, 0, 0.1 * (k + 1)]) for k in range(n_tris)])
+    tris[1] = tris[n_tris - 1] = base + np.float32([0, 0, 0.05])       # the nearest plane from below, twice
+    b = hcc_inputs.make_bvh([((0, 0, 0.05), (1, 1, 0.1 * n_tris), 0, n_tris)], tris)
+    rays = _rand_rays(513, 0x71E5)
+    rays[:, 0:3] = (0.2, 0.2, -1.0)
+    rays[:, 0:2] += 0.1 * rays[:, 4:6]
+    rays[:, 4:7] = (0.0, 0.0, 1.0)
+    want = _check_trace_both_modes(hcc, b, rays)
+    bvh = hcc.Bvh(b.nodes, b.tris, b.prim_idx)
+    t, prim, _, _ = hcc.hits_to_numpy(hcc.trace(bvh, torch.from_numpy(rays).cuda(), None, hcc.TRACE_CLOSEST))
+    assert np.all(~np.isinf(t)) and np.all(prim == 1) and np.array_equal(prim, want[1])
+    # from above the farthest plane is nearest; it is unique
+    rays[:, 2] = 2.0
+    rays[:, 6] = -1.0
+    want = _check_trace_both_modes(hcc, b, rays)
+    assert np.all(want[1] == n_tris - 2)
+
+
+def test_pair_call_orders_later_work_behind_both_batches(hcc, dev_cases):
+    """Work enqueued on the stream right after hcc_reorder_trace_pair sees the hits of BOTH batches.  The second traversal
+    kernel is a dependent launch that does not wait at entry; it must still not complete before the first (it waits before
+    exit).  Worst case: a long batch a and a tiny batch b, then a device-to-host copy of hits_a with nothing in between."""
+    d = dev_cases["room_mid"]
+    cut = hcc.select_cut(d["bvh"], hcc.density(d["bvh"]), 1024, 32)
+    ra = d["diffuse"].repeat(8, 1).contiguous()          # 524,288 closest-hit rays
+    rb = d["shadow"][:8].contiguous()
+    ref_a = hcc.trace(d["bvh"], ra, None, hcc.TRACE_CLOSEST)
+    ref_b = hcc.trace(d["bvh"], rb, None, hcc.TRACE_ANY)
+    ha, hb = torch.empty_like(ref_a), torch.empty_like(ref_b)
+    host_a = torch.empty(ref_a.shape, dtype=torch.float32).pin_memory()
+    pipe = hcc.Pipeline(ra.shape[0], 64, pair=True)
+    want = ref_a.cpu().view(torch.int32)
+    for order in (hcc.ORDER_HCC, hcc.ORDER_NOSORT):
+        for rep in range(5):
+            ha.fill_(-1.0); hb.fill_(7); host_a.fill_(-2.0)
+            pipe.reorder_trace_pair(d["bvh"], cut, order, ra, hcc.TRACE_CLOSEST, ha, rb, hcc.TRACE_ANY, hb)
+            host_a.copy_(ha, non_blocking=True)          # directly behind the call, same stream
+            torch.cuda.current_stream().synchronize()
+            assert torch.equal(host_a.view(torch.int32), want), (order, rep)
+            assert torch.equal(hb, ref_b)
+    pipe.close()
+
+
+def test_pipeline_synchronize_waits_for_the_last_call_of_any_form(hcc, dev_cases):
+    """hcc_pipeline_synchronize after a host-buffer call followed by a device-buffer call waits for the LATTER (the host
+    form's completion event must not be mistaken for it)."""
+    d = dev_cases["room_mid"]
+    cut = hcc.select_cut(d["bvh"], hcc.density(d["bvh"]), 1024, 32)
+    rays_h = d["case"].diffuse[:4096]
+    ra = d["diffuse"].repeat(16, 1).contiguous()         # about a millisecond of device work
+    ha = torch.empty((ra.shape[0], 4), dtype=torch.float32, device="cuda")
+    pipe = hcc.Pipeline(ra.shape[0], 64, host_staging=True)
+    hits_h = np.empty((4096, 4), dtype=np.float32)
+    s = torch.cuda.current_stream()
+    for rep in range(5):
+        pipe.reorder_trace_host(d["bvh"], cut, hcc.ORDER_HCC, rays_h, hits_h, hcc.TRACE_CLOSEST)
+        pipe.reorder_trace(d["bvh"], cut, hcc.ORDER_HCC, ra, hcc.TRACE_CLOSEST, hits=ha)
+        pipe.synchronize()
+        assert s.query(), rep                            # nothing of the device call is still running
+    pipe.close()
 
 
 def test_trace_deep_chain_bvh_spills_the_stack(hcc):
