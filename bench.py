@@ -607,17 +607,29 @@ def run_ours(args):
     by_bounce = {str(args.bounce): {"speedup_hcc": speed, "rays": n,
                                     "trace_ms": {o: {b_: orders[o][b_]["trace_ms"] for b_ in ("diffuse", "shadow")} for o in orders}}}
     shuffled = None
-    if world == 1 and args.bounces:
+    def warp_counters(sc_):
+        """Per batch and order: distinct node records and lanes per warp-level node step, node records per ray (hcc_trace_stats)."""
+        return {bn: {on: {k_: v_[k_] for k_ in ("distinct_records_per_warp_step", "lanes_per_warp_step", "node_records_per_ray", "tri_tests_per_ray")}
+                     for on, v_ in d_["orders"].items()} for bn, d_ in counters(sc_).items()}
+
+    def bounce_entry(sc_, o_b, s_b):
+        return {"speedup_hcc": s_b, "rays": sc_.n, "rays_diffuse": sc_.n_d, "rays_shadow": sc_.n_s,
+                "trace_ms": {o: {b_: o_b[o][b_]["trace_ms"] for b_ in ("diffuse", "shadow")} for o in o_b},
+                "encode_sort_ms": {o: {b_: o_b[o][b_]["encode_ms"] + o_b[o][b_]["sort_ms"] for b_ in ("diffuse", "shadow")} for o in o_b},
+                "incl_ms_per_step": {o: o_b[o]["ms_per_step"] for o in o_b},
+                "pair_ms_per_step": {o: o_b[o]["pair_ms_per_step"] for o in o_b},
+                "warp_counters": warp_counters(sc_)}
+
+    if world == 1 and args.bounces > 0:
+        by_bounce[str(args.bounce)] = bounce_entry(sc, orders, speed)
         k_b = max(3, min(args.steps, 10))
-        for b_i in range(args.bounce + 1, args.bounce + 3):
+        for b_i in range(args.bounce + 1, args.bounce + 1 + args.bounces):
             set_bounce(sc, b_i)
             o_b, s_b = compare(sc, k_b)
-            by_bounce[str(b_i)] = {"speedup_hcc": s_b, "rays": sc.n,
-                                   "trace_ms": {o: {b_: o_b[o][b_]["trace_ms"] for b_ in ("diffuse", "shadow")} for o in o_b}}
+            by_bounce[str(b_i)] = bounce_entry(sc, o_b, s_b)
         set_bounce(sc, args.bounce, shuffle=True)
         o_s, s_s = compare(sc, k_b)
-        shuffled = {"speedup_hcc": s_s, "trace_ms": {o: {b_: o_s[o][b_]["trace_ms"] for b_ in ("diffuse", "shadow")} for o in o_s},
-                    "incl_ms_per_step": {o: o_s[o]["ms_per_step"] for o in o_s},
+        shuffled = {**bounce_entry(sc, o_s, s_s),
                     "how": "the same two batches in a seeded random order (a wavefront renderer does not emit rays in camera order)"}
         set_bounce(sc, args.bounce)
         step(sc, hcc.ORDER_HCC)      # the hit buffers hold the unshuffled batches' results again (checked by the e2e leg)
@@ -898,7 +910,8 @@ def main():
     ap.add_argument("--large-n", action="store_true", help="the large-batch (33.5 M rays) encode/sort roofline leg")
     ap.add_argument("--no-large-n", dest="large_n", action="store_false", help="(default)")
     ap.add_argument("--configs", default="", help="comma list of further configs to run at their stated sizes (fig1,large): other_configs")
-    ap.add_argument("--bounces", action="store_true", help="the two later bounces and the shuffled-input leg of the workload")
+    ap.add_argument("--bounces", type=int, default=0,
+                    help="also run the three orders on this many LATER bounces of the workload and on its shuffled first batch (speedup_hcc_by_bounce, shuffled_input)")
     ap.add_argument("--full-json", default="", help="write the complete result (every section) to this file")
     ap.add_argument("--sections", action="store_true",
                     help="print every section of the result as its own JSON line before the final compact line")

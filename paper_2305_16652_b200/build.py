@@ -58,6 +58,20 @@ def build(force=False, verbose=False):
     return LIB
 
 
+def build_pipe_rates():
+    """The instruction-rate microbenchmark (csrc/pipe_rates.cu): a standalone debug program, not part of the library."""
+    out = os.path.join(_HERE, "pipe_rates")
+    cmd = [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+           os.path.join(CSRC, "pipe_rates.cu"), "-o", out]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed:\n" + r.stdout + r.stderr)
+    return out
+
+
 if __name__ == "__main__":
     import sys
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--pipe-rates" in sys.argv:
+        print(build_pipe_rates())
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
