@@ -50,7 +50,7 @@ OPS_BOX, OPS_NODE, OPS_TRI = 26, 68, 36
 # operations + 24 fma = 112 issue cycles' worth; per triangle test 10 compares/selects + 26 fma/mul/add = 46
 CYC_NODE, CYC_TRI = 2 * 44 + 24, 2 * 10 + 26
 SM_COUNT, LANES_PER_SM = 148, 128
-TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_trace_traffic.md")
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r3_trace_traffic.md")
 KERNEL_SOURCES = ("paper_2305_16652_b200/csrc/trace.cu", "paper_2305_16652_b200/csrc/bvh.cu",
                   "paper_2305_16652_b200/csrc/common.cuh")
 
@@ -70,7 +70,7 @@ def sort_bytes(key_b, passes):
 
 
 def kernel_source_hash():
-    """sha256 over the traversal kernel's sources: profiles/r2_trace_traffic.md records the hash its ncu capture
+    """sha256 over the traversal kernel's sources: profiles/r3_trace_traffic.md records the hash its ncu capture
     was taken at, so a stale capture is never reported (the GPU box has no .git to ask for HEAD)."""
     import hashlib
     h = hashlib.sha256()
@@ -596,7 +596,7 @@ def run_ours(args):
     roof = {"bound": roof["bound"], "achieved": roof["achieved"], "peak": roof["peak"], "unit": roof["unit"],
             "frac": roof["frac"],
             "traffic": ncu_traffic(args.workload, dom[0]) if plain else None,
-            "traffic_unit": "bytes per launch (dram read + write, ncu --set full; profiles/r2_trace_traffic.md, null when the "
+            "traffic_unit": "bytes per launch (dram read + write, ncu --set full; profiles/r3_trace_traffic.md, null when the "
                             "kernel sources changed since the capture)",
             "kernel": f"{dom[1]} ({dom[0]} batch)",
             "peak_source": (f"{peak_kind} HBM copy" if roof["bound"] == "hbm" else
