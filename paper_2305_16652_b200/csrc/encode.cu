@@ -145,7 +145,7 @@ constexpr int ENC_HCC_THREADS = 1024;
 
 // Alg. 1: line 1 "copy cut nodes from global memory into shared memory" (the first
 // smem_entries entries = whole levels), line 2 grid-stride "while have ray", lines 4-6 per
-// level.  One ray per thread per iteration; 32-byte rays read as two 16-byte loads.
+// level.  One ray per thread per iteration; a 32-byte ray is read with ONE 256-bit load (ld.global.nc.v8.f32).
 template <typename KeyT>
 __global__ void __launch_bounds__(ENC_HCC_THREADS, 1)
 k_encode_hcc(const float4 *__restrict__ rays, uint64_t n, const CutDev cut, uint32_t smem_entries,

@@ -42,7 +42,7 @@ constexpr int HIST_BATCH = HCC_HIST_BATCH;
 constexpr float MATCH_MAX_DISTINCT = (float)HCC_SORT_FEW;   // expected distinct digits per warp up to which MATCH.ANY is used
 constexpr int LOOK = 4;                      // look-back rows fetched per round trip
 
-// control region of the workspace (zeroed once per sort by one memset)
+// control region of the workspace (zeroed at the start of every sort by k_sort_init, the first kernel of its chain)
 struct SortCtl {
     uint32_t hist[MAX_PASSES][RADIX];
     uint32_t ticket[MAX_PASSES];
